@@ -1,0 +1,234 @@
+/*
+ * swiftcache.h -- C ABI of the B200-native SwiftCache multi-turn prefill hot path.
+ *
+ * What the library does (arxiv/paper_2606_16135, cited as PAPER.md:<line>):
+ * for each transformer layer in turn, the conversation's historical KV is
+ * fetched from a paged block pool through a block table into a small
+ * active-layer buffer (the "layer stream cache", LSC, Sec. 3.2),
+ * the turn's new tokens run causal attention over that history plus
+ * themselves (Sec. 2.2), and their fresh K/V are scattered
+ * back into pool blocks (Sec. 3.3).  Only the current
+ * layer's KV, double-buffered, is resident in the LSC.
+ *
+ * Conventions
+ *   - Plain C, no torch / C++ types.  Every pointer says HOST or DEVICE.
+ *   - bf16 tensors are passed as `const void*` to raw bf16 bits.
+ *   - Streams are passed as `void*` holding a cudaStream_t (0 = default stream).
+ *   - Every call returns sc_status_t; SC_OK is 0.  sc_last_error() gives a
+ *     thread-local message for the last failing call.  Argument errors are
+ *     detected on the host before any launch; nothing is launched on error.
+ *   - Data calls only ENQUEUE work on the given stream and return.  Ordering
+ *     between different streams is the caller's job (or the pipeline
+ *     helper's, sc_prefill_turn).
+ *   - Ownership: the sc_pool_t object and its internal scratch belong to the
+ *     library.  pool_base / lsc_base and every tensor or table pointer are
+ *     BORROWED from the caller and never freed here (the pool is *donated*
+ *     memory in the paper too).
+ *
+ * Pool geometry ("block-major layout", Eq. 1)
+ *   pool  = [n_blocks][n_layers] cells, each cell M_block = 2*B*Hkv*D*2 bytes
+ *   cell  = [kv: K,V][Hkv] chunks, each chunk = the B=16 tokens x D values of
+ *           one head, B*D*2 bytes, contiguous
+ *   chunk = stored in the tensor core's 128-byte-swizzled operand order so a
+ *           chunk is usable as a tcgen05.mma shared-memory operand after ONE
+ *           contiguous bulk copy.  Byte offset of (slot s, dim d) in a chunk:
+ *             (s/8)*(D/64)*1024 + (d/64)*1024 + (s%8)*128
+ *               + ((((d%64)/8) ^ (s%8)) * 16) + (d%8)*2
+ *           sc_cell_offset() returns the full byte offset; tests use it as
+ *           the logical accessor.  The paper leaves the in-block order open
+ *           (reading S3 in DESIGN.md).
+ *   LSC   = 2 buffers x lsc_blocks cells in LOGICAL block order, same cell
+ *           format, so a layer load is one contiguous M_block copy per block.
+ */
+#ifndef SWIFTCACHE_H_
+#define SWIFTCACHE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sc_pool sc_pool_t; /* opaque, owned by the library */
+
+typedef enum {
+    SC_OK = 0,
+    SC_ERR_INVALID_ARG = 1,   /* null pointer, negative size, layer out of range ...        */
+    SC_ERR_OUT_OF_BLOCKS = 2, /* allocator exhausted; nothing was allocated                 */
+    SC_ERR_CAPACITY = 3,      /* table / LSC / scratch too small for the request            */
+    SC_ERR_BAD_BLOCK_ID = 4,  /* id out of range, double free, or not allocated             */
+    SC_ERR_CUDA = 5,          /* a CUDA runtime call failed (also: no device present)       */
+    SC_ERR_UNSUPPORTED = 6    /* head_dim not in {64,128}, block_size != 16, Hq % Hkv != 0  */
+} sc_status_t;
+
+typedef enum { SC_POOL_HBM = 0, SC_POOL_HOST_PINNED = 1 } sc_pool_kind_t;
+typedef enum { SC_ATTN_STAGED = 0, SC_ATTN_FUSED = 1 } sc_attn_mode_t;
+typedef enum { SC_MEM_DEVICE = 0, SC_MEM_HOST_PINNED = 1 } sc_mem_kind_t;
+/* which attention engine sc_prefill_layer* uses; AUTO picks the fastest one
+ * that supports the shape */
+typedef enum { SC_ENGINE_AUTO = 0, SC_ENGINE_MMA_SYNC = 1, SC_ENGINE_TCGEN05 = 2 } sc_engine_t;
+/* which copy engine sc_load_layer* uses */
+typedef enum { SC_COPY_AUTO = 0, SC_COPY_LDG = 1, SC_COPY_BULK = 2 } sc_copy_t;
+
+typedef struct {
+    int32_t n_layers;       /* L                                                          */
+    int32_t n_q_heads;      /* Hq                                                         */
+    int32_t n_kv_heads;     /* Hkv, must divide Hq                                        */
+    int32_t head_dim;       /* D, 64 or 128                                               */
+    int32_t block_size;     /* B tokens per block, must be 16                             */
+    int32_t n_blocks;       /* pool capacity in full-layer blocks                         */
+    int32_t pool_kind;      /* sc_pool_kind_t: where pool_base lives                      */
+    int32_t lsc_blocks;     /* capacity of EACH of the two LSC buffers, in blocks         */
+    int32_t max_new_tokens; /* most new tokens (summed over a batch) in one prefill call  */
+    int32_t max_seqs;       /* most conversations in one batched call (>= 1)              */
+    uint64_t alloc_seed;    /* 0: free list hands out ascending ids; else seeded shuffle  */
+} sc_pool_config_t;
+
+typedef struct {
+    int64_t chunk_bytes;      /* B*D*2                                                    */
+    int64_t cell_bytes;       /* M_block of Eq. 1 = 2*Hkv*chunk_bytes                     */
+    int64_t block_bytes;      /* n_layers*cell_bytes: stride between pool blocks          */
+    int64_t pool_bytes;       /* n_blocks*block_bytes                                     */
+    int64_t lsc_buffer_bytes; /* lsc_blocks*cell_bytes: one of the two LSC buffers        */
+    int64_t lsc_bytes;        /* 2*lsc_buffer_bytes                                       */
+    int64_t scratch_bytes;    /* device scratch the library allocated for itself          */
+    int32_t n_free_blocks;
+    int32_t max_splits;       /* most split-KV partitions the attention may use           */
+} sc_pool_info_t;
+
+/* ------------------------------------------------------------------ lifecycle */
+
+const char *sc_version(void);
+/* Thread-local, static storage; valid until the next failing call on this thread. */
+const char *sc_last_error(void);
+
+/* Bytes the caller must provide for the pool region and for the LSC region (both
+ * LSC buffers).  Pure host arithmetic (Eq. 1); works without a GPU.  HOST pointers. */
+sc_status_t sc_pool_bytes_required(const sc_pool_config_t *cfg, size_t *pool_bytes, size_t *lsc_bytes);
+
+/* pool_base: DEVICE pointer (SC_POOL_HBM) or pinned, device-mapped HOST pointer
+ * (SC_POOL_HOST_PINNED), 1024-byte aligned, >= pool_bytes.  lsc_base: DEVICE pointer,
+ * 1024-byte aligned, >= lsc_bytes; may be NULL with lsc_blocks == 0 (fused mode only).
+ * If zero_fill != 0 both regions are cleared (S10: slots never written must hold
+ * finite values).  Passing pool_base == NULL creates a HOST-ONLY pool object: the
+ * allocator / block-table calls work, every data call fails with SC_ERR_CUDA.       */
+sc_status_t sc_pool_create(const sc_pool_config_t *cfg, void *pool_base, size_t pool_bytes,
+                           void *lsc_base, size_t lsc_bytes, int32_t zero_fill, sc_pool_t **out);
+sc_status_t sc_pool_destroy(sc_pool_t *pool);
+sc_status_t sc_pool_info(const sc_pool_t *pool, sc_pool_info_t *info /* HOST */);
+
+/* Logical accessor: byte offset from pool_base of element (block, layer, kv, head,
+ * slot, d); kv = 0 for K, 1 for V.  *offset HOST.  Pure host arithmetic.            */
+sc_status_t sc_cell_offset(const sc_pool_t *pool, int32_t block, int32_t layer, int32_t kv,
+                           int32_t head, int32_t slot, int32_t d, int64_t *offset);
+/* Same for the LSC: byte offset from lsc_base of (buf, logical block, kv, head, slot, d). */
+sc_status_t sc_lsc_offset(const sc_pool_t *pool, int32_t buf, int32_t lblock, int32_t kv,
+                          int32_t head, int32_t slot, int32_t d, int64_t *offset);
+
+/* Select engines (defaults: AUTO).  Takes effect for later calls. */
+sc_status_t sc_set_engine(sc_pool_t *pool, int32_t attn_engine /* sc_engine_t */,
+                          int32_t copy_engine /* sc_copy_t */);
+/* Force the number of split-KV tiles per partition (0 = automatic). */
+sc_status_t sc_set_split_tiles(sc_pool_t *pool, int32_t tiles_per_split);
+
+/* ------------------------------------------------- a1/a2: allocator and block tables
+ * PAPER.md:142 (block table), :214-216 (block-major pool).  All arrays HOST.          */
+
+/* All-or-nothing: on SC_ERR_OUT_OF_BLOCKS nothing is allocated.  Ids are distinct,
+ * in [0, n_blocks), and were free (S15: which ids is unspecified).                    */
+sc_status_t sc_alloc_blocks(sc_pool_t *pool, int32_t n, int32_t *ids_out);
+/* SC_ERR_BAD_BLOCK_ID (and nothing freed) if any id is out of range, not allocated,
+ * or repeated in the list.                                                            */
+sc_status_t sc_free_blocks(sc_pool_t *pool, const int32_t *ids, int32_t n);
+sc_status_t sc_num_free_blocks(const sc_pool_t *pool, int32_t *n_free);
+/* Grow `table` (HOST array of capacity `cap`, currently *n_table entries) so that it
+ * covers hist_len + n_new tokens: appends ceil((hist_len+n_new)/B) - *n_table fresh
+ * ids (>= 0 of them).  Requires *n_table >= ceil(hist_len/B).  SC_ERR_CAPACITY if cap
+ * is too small, SC_ERR_OUT_OF_BLOCKS if the pool is; in both cases nothing changes.   */
+sc_status_t sc_append_blocks(sc_pool_t *pool, int32_t *table, int32_t *n_table, int32_t cap,
+                             int32_t hist_len, int32_t n_new);
+
+/* ------------------------------------------------------------------ data calls
+ * Shapes use n = tokens, Hq/Hkv/D from the config.  "packed" means the sequences of
+ * a batch are concatenated along the token axis.  SC_MAX_SEQS bounds a batch.       */
+#define SC_MAX_SEQS 32
+
+/* a3 -- PAPER.md:190 ("KV Store").  k, v: DEVICE bf16 [n_tokens][Hkv][D] of ONE layer,
+ * written at logical tokens [start_token, start_token + n_tokens) of the conversation
+ * whose table is table_dev (DEVICE int32[n_table], must cover the range).  Byte-exact. */
+sc_status_t sc_store_prefix(sc_pool_t *pool, int32_t layer, const void *k, const void *v,
+                            int32_t start_token, int32_t n_tokens, const int32_t *table_dev,
+                            int32_t n_table, void *stream);
+
+/* Inverse of a3, for verification and for callers that want contiguous KV back:
+ * k_out, v_out DEVICE bf16 [n_tokens][Hkv][D] <- logical tokens [start, start+n).
+ * src = 0: the pool through table_dev; src = 1 / 2: LSC buffer 0 / 1 (table_dev
+ * ignored, logical block j is LSC block lsc_block_off + j).  Byte-exact.              */
+sc_status_t sc_read_tokens(sc_pool_t *pool, int32_t layer, int32_t src, const int32_t *table_dev,
+                           int32_t n_table, int32_t lsc_block_off, int32_t start_token,
+                           int32_t n_tokens, void *k_out, void *v_out, void *stream);
+
+/* a4 -- PAPER.md:148, :192 ("KV Load"): paged gather pool -> LSC[buf] of this layer's
+ * first ceil(hist_len/B) blocks, in logical order (whole blocks are copied; S10).
+ * SC_ERR_CAPACITY if they do not fit in lsc_blocks.  Enqueued on `stream` (the copy
+ * stream).  The caller orders it before the sc_prefill_layer(STAGED) that reads buf
+ * and after the previous reader of buf.                                               */
+sc_status_t sc_load_layer(sc_pool_t *pool, int32_t layer, const int32_t *table_dev,
+                          int32_t n_table, int32_t hist_len, int32_t buf, void *stream);
+
+/* a5+a6+a7 -- PAPER.md:148, :190 (scatter), :72, :87 (attention).
+ * q, out: DEVICE bf16 [n_new][Hq][D];  k_new, v_new: DEVICE bf16 [n_new][Hkv][D].
+ * table_dev: DEVICE int32[n_table] covering hist_len + n_new tokens (sc_append_blocks).
+ * Steps, all enqueued on `stream`:
+ *   1. scatter k_new/v_new to logical tokens hist_len.. of the pool (and, in STAGED
+ *      mode, to the same logical positions of LSC[buf]);
+ *   2. out[i,h,:] = sum_j softmax_j(q[i,h].K[j,h/G]/sqrt(D)) V[j,h/G,:], j <= hist_len+i,
+ *      K/V = [history ; new], bf16 inputs, fp32 accumulation, bf16 output;
+ *      STAGED reads LSC[buf] (history must have been loaded there), FUSED reads the
+ *      pool blocks directly through table_dev and ignores buf;
+ *   3. if the history was split across CTAs, the partial (m, l, O) triples are merged.
+ * SC_ERR_CAPACITY: table too short, LSC too small (STAGED), n_new > max_new_tokens.    */
+sc_status_t sc_prefill_layer(sc_pool_t *pool, int32_t layer, const void *q, const void *k_new,
+                             const void *v_new, const int32_t *table_dev, int32_t n_table,
+                             int32_t hist_len, int32_t n_new, int32_t buf, int32_t mode,
+                             void *out, void *stream);
+
+/* a9 -- ragged batch (continuous batching is assumed by the paper).
+ * tables_dev: DEVICE int32 [n_seq][max_blocks] (entries past a sequence's table are
+ * ignored).  hist_lens, cu_new: HOST int32 [n_seq], [n_seq+1] (cu_new[0] = 0, new
+ * tokens of sequence s are rows cu_new[s]..cu_new[s+1]-1 of the packed tensors).
+ * In the LSC, sequence s starts at block sum_{t<s} ceil((hist_lens[t]+n_new[t])/B).    */
+sc_status_t sc_load_layer_batched(sc_pool_t *pool, int32_t layer, const int32_t *tables_dev,
+                                  int32_t max_blocks, int32_t n_seq, const int32_t *hist_lens,
+                                  const int32_t *cu_new, int32_t buf, void *stream);
+sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void *q,
+                                     const void *k_new, const void *v_new,
+                                     const int32_t *tables_dev, int32_t max_blocks, int32_t n_seq,
+                                     const int32_t *hist_lens, const int32_t *cu_new, int32_t buf,
+                                     int32_t mode, void *out, void *stream);
+
+/* a8 -- the layer-streaming pipeline of one turn (ordering rule :192),
+ * with the two-buffer reading S8 of DESIGN.md: for l = 0..L-1, the copy stream loads
+ * layer l+1 into LSC[(l+1)%2] while the compute stream scatters + attends layer l from
+ * LSC[l%2]; load(l+1) waits for attention(l-1), attention(l) waits for load(l).
+ * Layers are issued strictly in order, one sc_prefill_layer_batched per layer.
+ * q_all, out_all: [L][sum n_new][Hq][D]; k_all, v_all: [L][sum n_new][Hkv][D], bf16.
+ * io_kind (sc_mem_kind_t): SC_MEM_DEVICE = DEVICE pointers; SC_MEM_HOST_PINNED = pinned
+ * HOST pointers, in which case each layer's q/k/v are copied host->device and its out
+ * device->host inside the call (double-buffered staging owned by the library).
+ * mode FUSED skips the loads.  On return all work is enqueued; compute_stream has been
+ * made to wait for everything (synchronise it to wait for the turn).                   */
+sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_all,
+                            const void *v_all, void *out_all, int32_t io_kind,
+                            const int32_t *tables_dev, int32_t max_blocks, int32_t n_seq,
+                            const int32_t *hist_lens, const int32_t *cu_new, int32_t mode,
+                            void *copy_stream, void *compute_stream);
+
+/* Number of kernels the library has launched since the pool was created (all kinds). */
+sc_status_t sc_launch_count(const sc_pool_t *pool, int64_t *n_launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SWIFTCACHE_H_ */

@@ -1,0 +1,350 @@
+// sc_ops.cu -- the data calls of the C ABI (a3-a9): argument checking on the host,
+// then kernel launches on the caller's stream.  No step of the path runs on the CPU.
+#include <string.h>
+
+#include "sc_internal.h"
+
+namespace {
+
+#define SC_CUDA(call)                                                   \
+    do {                                                                \
+        cudaError_t e_ = (call);                                        \
+        if (e_ != cudaSuccess) return sc_cuda_fail(e_, #call);          \
+    } while (0)
+
+inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+sc_status_t check_pool(sc_pool_t *p, int32_t layer)
+{
+    if (!p) return sc_fail(SC_ERR_INVALID_ARG, "pool is NULL");
+    if (p->host_only) return sc_fail(SC_ERR_CUDA, "host-only pool (created without memory): no data calls");
+    if (layer < 0 || layer >= p->g.L) return sc_fail(SC_ERR_INVALID_ARG, "layer %d not in [0,%d)", layer, p->g.L);
+    return SC_OK;
+}
+
+ScKvView pool_view(const sc_pool_t *p, int layer, const int32_t *tables, int max_blocks)
+{
+    ScKvView v;
+    v.base = p->pool_base + (int64_t)layer * p->g.cell_bytes;
+    v.block_stride = p->g.block_bytes;
+    v.tables = tables;
+    v.max_blocks = max_blocks;
+    return v;
+}
+
+ScKvView lsc_view(const sc_pool_t *p, int buf)
+{
+    ScKvView v;
+    v.base = p->lsc_base + (int64_t)buf * p->lsc_buffer_bytes;
+    v.block_stride = p->g.cell_bytes;
+    v.tables = nullptr;
+    v.max_blocks = 0;
+    return v;
+}
+
+// Validates a ragged batch and fills the by-value descriptor.  `with_new` = 0 for the
+// gather (blocks to copy = ceil(hist/B)), but LSC offsets always reserve room for the
+// new tokens so load and prefill agree on the placement.
+sc_status_t make_batch(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, const int32_t *cu_new,
+                       int max_blocks, int tile_m, ScBatch *b)
+{
+    if (n_seq <= 0 || n_seq > p->cfg.max_seqs) return sc_fail(SC_ERR_CAPACITY, "n_seq %d not in [1,%d]", n_seq, p->cfg.max_seqs);
+    if (!hist_lens || !cu_new) return sc_fail(SC_ERR_INVALID_ARG, "hist_lens / cu_new is NULL");
+    if (cu_new[0] != 0) return sc_fail(SC_ERR_INVALID_ARG, "cu_new[0] != 0");
+    memset(b, 0, sizeof *b);
+    b->n_seq = n_seq;
+    int lsc = 0, mt = 0, blk = 0;
+    for (int s = 0; s < n_seq; ++s) {
+        const int n = cu_new[s + 1] - cu_new[s];
+        if (hist_lens[s] < 0 || n < 0) return sc_fail(SC_ERR_INVALID_ARG, "negative length in sequence %d", s);
+        const int64_t tot = (int64_t)hist_lens[s] + n;
+        if (tot > (int64_t)max_blocks * p->g.B)
+            return sc_fail(SC_ERR_CAPACITY, "sequence %d: %lld tokens exceed table of %d blocks", s, (long long)tot, max_blocks);
+        b->hist[s] = hist_lens[s];
+        b->cu_new[s] = cu_new[s];
+        b->lsc_off[s] = lsc;
+        b->cu_mt[s] = mt;
+        b->cu_blk[s] = blk;
+        lsc += ceil_div((int)tot, p->g.B);
+        mt += ceil_div(n, tile_m);
+        blk += ceil_div(hist_lens[s], p->g.B);
+    }
+    b->cu_new[n_seq] = cu_new[n_seq];
+    b->cu_mt[n_seq] = mt;
+    b->cu_blk[n_seq] = blk;
+    for (int s = n_seq; s < SC_MAX_SEQS; ++s) b->lsc_off[s] = lsc;   // total, read by callers
+    if (cu_new[n_seq] > p->cfg.max_new_tokens)
+        return sc_fail(SC_ERR_CAPACITY, "%d new tokens > max_new_tokens %d", cu_new[n_seq], p->cfg.max_new_tokens);
+    return SC_OK;
+}
+
+int lsc_blocks_needed(const ScBatch &b) { return b.lsc_off[SC_MAX_SEQS - 1]; }
+
+}  // namespace
+
+extern "C" {
+
+sc_status_t sc_store_prefix(sc_pool_t *pool, int32_t layer, const void *k, const void *v,
+                            int32_t start_token, int32_t n_tokens, const int32_t *table_dev,
+                            int32_t n_table, void *stream)
+{
+    sc_status_t st = check_pool(pool, layer);
+    if (st) return st;
+    if (start_token < 0 || n_tokens < 0) return sc_fail(SC_ERR_INVALID_ARG, "negative token range");
+    if (n_tokens == 0) return SC_OK;
+    if (!k || !v || !table_dev) return sc_fail(SC_ERR_INVALID_ARG, "NULL tensor or table");
+    if ((int64_t)start_token + n_tokens > (int64_t)n_table * pool->g.B)
+        return sc_fail(SC_ERR_CAPACITY, "tokens [%d,%d) exceed table of %d blocks", start_token,
+                       start_token + n_tokens, n_table);
+    ScBatch b;
+    memset(&b, 0, sizeof b);
+    b.n_seq = 1;
+    b.hist[0] = start_token;
+    b.cu_new[1] = n_tokens;
+    SC_CUDA(sc_launch_scatter(pool->g, k, v, b, pool_view(pool, layer, table_dev, n_table), nullptr,
+                              (cudaStream_t)stream));
+    pool->launches += 1;
+    return SC_OK;
+}
+
+sc_status_t sc_read_tokens(sc_pool_t *pool, int32_t layer, int32_t src, const int32_t *table_dev,
+                           int32_t n_table, int32_t lsc_block_off, int32_t start_token,
+                           int32_t n_tokens, void *k_out, void *v_out, void *stream)
+{
+    sc_status_t st = check_pool(pool, layer);
+    if (st) return st;
+    if (start_token < 0 || n_tokens < 0 || src < 0 || src > 2) return sc_fail(SC_ERR_INVALID_ARG, "bad range or src");
+    if (n_tokens == 0) return SC_OK;
+    if (!k_out || !v_out) return sc_fail(SC_ERR_INVALID_ARG, "NULL output");
+    ScBatch b;
+    memset(&b, 0, sizeof b);
+    b.n_seq = 1;
+    b.hist[0] = start_token;
+    b.cu_new[1] = n_tokens;
+    ScKvView view;
+    if (src == 0) {
+        if (!table_dev) return sc_fail(SC_ERR_INVALID_ARG, "table is NULL");
+        if ((int64_t)start_token + n_tokens > (int64_t)n_table * pool->g.B)
+            return sc_fail(SC_ERR_CAPACITY, "tokens exceed table of %d blocks", n_table);
+        view = pool_view(pool, layer, table_dev, n_table);
+    } else {
+        if (!pool->lsc_base) return sc_fail(SC_ERR_CAPACITY, "pool has no LSC");
+        const int last = lsc_block_off + ceil_div(start_token + n_tokens, pool->g.B);
+        if (lsc_block_off < 0 || last > pool->cfg.lsc_blocks)
+            return sc_fail(SC_ERR_CAPACITY, "tokens exceed the LSC (%d blocks)", pool->cfg.lsc_blocks);
+        view = lsc_view(pool, src - 1);
+        b.lsc_off[0] = lsc_block_off;
+    }
+    SC_CUDA(sc_launch_read(pool->g, k_out, v_out, b, view, (cudaStream_t)stream));
+    pool->launches += 1;
+    return SC_OK;
+}
+
+sc_status_t sc_load_layer_batched(sc_pool_t *pool, int32_t layer, const int32_t *tables_dev,
+                                  int32_t max_blocks, int32_t n_seq, const int32_t *hist_lens,
+                                  const int32_t *cu_new, int32_t buf, void *stream)
+{
+    sc_status_t st = check_pool(pool, layer);
+    if (st) return st;
+    if (!tables_dev || max_blocks <= 0) return sc_fail(SC_ERR_INVALID_ARG, "bad table");
+    if (buf < 0 || buf > 1) return sc_fail(SC_ERR_INVALID_ARG, "buf %d not in {0,1}", buf);
+    ScBatch b;
+    st = make_batch(pool, n_seq, hist_lens, cu_new, max_blocks, sc_mma_tile_m(), &b);
+    if (st) return st;
+    if (!pool->lsc_base || lsc_blocks_needed(b) > pool->cfg.lsc_blocks)
+        return sc_fail(SC_ERR_CAPACITY, "batch needs %d LSC blocks, buffer holds %d", lsc_blocks_needed(b),
+                       pool->cfg.lsc_blocks);
+    int engine = pool->copy_engine;
+    if (engine == SC_COPY_AUTO) engine = SC_COPY_LDG;
+    SC_CUDA(sc_launch_gather(pool->g, b, pool_view(pool, layer, tables_dev, max_blocks), lsc_view(pool, buf),
+                             engine, pool->n_sms, (cudaStream_t)stream));
+    pool->launches += (b.cu_blk[n_seq] > 0);
+    return SC_OK;
+}
+
+sc_status_t sc_load_layer(sc_pool_t *pool, int32_t layer, const int32_t *table_dev, int32_t n_table,
+                          int32_t hist_len, int32_t buf, void *stream)
+{
+    // reserve nothing for new tokens here: the single-sequence LSC always starts at block 0
+    const int32_t cu[2] = {0, 0};
+    if (pool && hist_len > (int64_t)n_table * pool->g.B)
+        return sc_fail(SC_ERR_CAPACITY, "hist_len %d exceeds table of %d blocks", hist_len, n_table);
+    return sc_load_layer_batched(pool, layer, table_dev, n_table, 1, &hist_len, cu, buf, stream);
+}
+
+sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void *q, const void *k_new,
+                                     const void *v_new, const int32_t *tables_dev, int32_t max_blocks,
+                                     int32_t n_seq, const int32_t *hist_lens, const int32_t *cu_new,
+                                     int32_t buf, int32_t mode, void *out, void *stream)
+{
+    sc_status_t st = check_pool(pool, layer);
+    if (st) return st;
+    if (!q || !k_new || !v_new || !out || !tables_dev || max_blocks <= 0)
+        return sc_fail(SC_ERR_INVALID_ARG, "NULL tensor or table");
+    if (mode != SC_ATTN_STAGED && mode != SC_ATTN_FUSED) return sc_fail(SC_ERR_INVALID_ARG, "mode %d", mode);
+    if (buf < 0 || buf > 1) return sc_fail(SC_ERR_INVALID_ARG, "buf %d not in {0,1}", buf);
+    int engine = pool->attn_engine;
+    if (engine == SC_ENGINE_AUTO) engine = SC_ENGINE_MMA_SYNC;
+    if (engine == SC_ENGINE_TCGEN05) return sc_fail(SC_ERR_UNSUPPORTED, "tcgen05 engine not built");
+    const int tile_m = sc_mma_tile_m(), tile_n = sc_mma_tile_n();
+    ScBatch b;
+    st = make_batch(pool, n_seq, hist_lens, cu_new, max_blocks, tile_m, &b);
+    if (st) return st;
+    const int total_new = b.cu_new[n_seq];
+    if (total_new == 0) return SC_OK;
+    const bool staged = (mode == SC_ATTN_STAGED);
+    if (staged && (!pool->lsc_base || lsc_blocks_needed(b) > pool->cfg.lsc_blocks))
+        return sc_fail(SC_ERR_CAPACITY, "batch needs %d LSC blocks, buffer holds %d", lsc_blocks_needed(b),
+                       pool->cfg.lsc_blocks);
+    cudaStream_t s = (cudaStream_t)stream;
+    const ScKvView pv = pool_view(pool, layer, tables_dev, max_blocks);
+    const ScKvView lv = staged ? lsc_view(pool, buf) : pv;
+
+    // 1. scatter (a5): pool, and the LSC tail in staged mode
+    SC_CUDA(sc_launch_scatter(pool->g, k_new, v_new, b, pv, staged ? &lv : nullptr, s));
+    pool->launches += 1;
+
+    // 2. attention (a6), split over the keys when that is needed to fill the machine
+    int max_tiles = 1;
+    for (int i = 0; i < n_seq; ++i)
+        max_tiles = std::max(max_tiles, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), tile_n));
+    const int base_ctas = pool->g.Hq * b.cu_mt[n_seq];
+    int split_tiles = pool->split_tiles_override;
+    if (split_tiles <= 0) {
+        int want = ceil_div(3 * pool->n_sms, base_ctas);
+        want = std::max(1, std::min(want, pool->max_splits));
+        split_tiles = std::max(ceil_div(max_tiles, want), 4);
+    }
+    int n_splits = ceil_div(max_tiles, split_tiles);
+    if (n_splits > pool->max_splits) {
+        split_tiles = ceil_div(max_tiles, pool->max_splits);
+        n_splits = ceil_div(max_tiles, split_tiles);
+    }
+    ScAttnArgs a;
+    a.q = q;
+    a.out = out;
+    a.kv = lv;
+    a.part_o = pool->part_o;
+    a.part_ml = pool->part_ml;
+    a.split_tiles = split_tiles;
+    a.n_splits = n_splits;
+    a.total_new = total_new;
+    SC_CUDA(sc_launch_attn_mma(pool->g, b, a, s));
+    pool->launches += 1;
+    // 3. combine (a7)
+    if (n_splits > 1) {
+        SC_CUDA(sc_launch_combine(pool->g, b, a, tile_m, tile_n, s));
+        pool->launches += 1;
+    }
+    return SC_OK;
+}
+
+sc_status_t sc_prefill_layer(sc_pool_t *pool, int32_t layer, const void *q, const void *k_new,
+                             const void *v_new, const int32_t *table_dev, int32_t n_table,
+                             int32_t hist_len, int32_t n_new, int32_t buf, int32_t mode, void *out,
+                             void *stream)
+{
+    if (n_new < 0) return sc_fail(SC_ERR_INVALID_ARG, "n_new < 0");
+    const int32_t cu[2] = {0, n_new};
+    return sc_prefill_layer_batched(pool, layer, q, k_new, v_new, table_dev, n_table, 1, &hist_len, cu,
+                                    buf, mode, out, stream);
+}
+
+sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_all, const void *v_all,
+                            void *out_all, int32_t io_kind, const int32_t *tables_dev,
+                            int32_t max_blocks, int32_t n_seq, const int32_t *hist_lens,
+                            const int32_t *cu_new, int32_t mode, void *copy_stream, void *compute_stream)
+{
+    sc_status_t st = check_pool(pool, 0);
+    if (st) return st;
+    if (!q_all || !k_all || !v_all || !out_all) return sc_fail(SC_ERR_INVALID_ARG, "NULL tensor");
+    if (io_kind != SC_MEM_DEVICE && io_kind != SC_MEM_HOST_PINNED) return sc_fail(SC_ERR_INVALID_ARG, "io_kind %d", io_kind);
+    if (mode != SC_ATTN_STAGED && mode != SC_ATTN_FUSED) return sc_fail(SC_ERR_INVALID_ARG, "mode %d", mode);
+    ScBatch b;
+    st = make_batch(pool, n_seq, hist_lens, cu_new, max_blocks, sc_mma_tile_m(), &b);   // validate early
+    if (st) return st;
+    const bool staged = (mode == SC_ATTN_STAGED);
+    if (staged && copy_stream == compute_stream)
+        return sc_fail(SC_ERR_INVALID_ARG, "staged mode needs two different streams");
+    cudaStream_t cs = (cudaStream_t)copy_stream, xs = (cudaStream_t)compute_stream;
+    const ScGeom &g = pool->g;
+    const int L = g.L, total_new = cu_new[n_seq];
+    const int64_t q_bytes = (int64_t)total_new * g.Hq * g.D * 2, kv_bytes = (int64_t)total_new * g.Hkv * g.D * 2;
+    const bool host_io = (io_kind == SC_MEM_HOST_PINNED);
+    if (host_io) {
+        const int64_t need = 2 * q_bytes + 2 * kv_bytes;   // q, out, k, v
+        if (pool->stage_bytes < need) {
+            for (int i = 0; i < 2; ++i) {
+                if (pool->stage[i]) cudaFree(pool->stage[i]);
+                pool->stage[i] = nullptr;
+            }
+            pool->stage_bytes = 0;
+            for (int i = 0; i < 2; ++i) SC_CUDA(cudaMalloc((void **)&pool->stage[i], (size_t)need));
+            pool->stage_bytes = need;
+        }
+    }
+    // fork: the side streams start after whatever the compute stream already holds
+    SC_CUDA(cudaEventRecord(pool->ev_fork, xs));
+    if (staged) {
+        SC_CUDA(cudaStreamWaitEvent(cs, pool->ev_fork, 0));
+        st = sc_load_layer_batched(pool, 0, tables_dev, max_blocks, n_seq, hist_lens, cu_new, 0, cs);
+        if (st) return st;
+        SC_CUDA(cudaEventRecord(pool->ev_load[0], cs));
+    }
+    if (host_io) {
+        SC_CUDA(cudaStreamWaitEvent(pool->h2d_stream, pool->ev_fork, 0));
+        SC_CUDA(cudaStreamWaitEvent(pool->d2h_stream, pool->ev_fork, 0));
+    }
+    for (int l = 0; l < L; ++l) {
+        const int bf = l & 1;
+        const char *q = (const char *)q_all + (int64_t)l * q_bytes;
+        const char *k = (const char *)k_all + (int64_t)l * kv_bytes;
+        const char *v = (const char *)v_all + (int64_t)l * kv_bytes;
+        char *o = (char *)out_all + (int64_t)l * q_bytes;
+        if (staged && l + 1 < L) {
+            // load(l+1) overwrites LSC[bf^1], last read by attention(l-1)
+            if (l >= 1) SC_CUDA(cudaStreamWaitEvent(cs, pool->ev_attn[bf ^ 1], 0));
+            st = sc_load_layer_batched(pool, l + 1, tables_dev, max_blocks, n_seq, hist_lens, cu_new, bf ^ 1, cs);
+            if (st) return st;
+            SC_CUDA(cudaEventRecord(pool->ev_load[bf ^ 1], cs));
+        }
+        const char *dq = q, *dk = k, *dv = v;
+        char *dout = o;
+        if (host_io) {
+            char *sb = pool->stage[bf];
+            if (l >= 2) SC_CUDA(cudaStreamWaitEvent(pool->h2d_stream, pool->ev_comp[bf], 0));
+            SC_CUDA(cudaMemcpyAsync(sb, q, (size_t)q_bytes, cudaMemcpyHostToDevice, pool->h2d_stream));
+            SC_CUDA(cudaMemcpyAsync(sb + q_bytes, k, (size_t)kv_bytes, cudaMemcpyHostToDevice, pool->h2d_stream));
+            SC_CUDA(cudaMemcpyAsync(sb + q_bytes + kv_bytes, v, (size_t)kv_bytes, cudaMemcpyHostToDevice, pool->h2d_stream));
+            SC_CUDA(cudaEventRecord(pool->ev_h2d[bf], pool->h2d_stream));
+            SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_h2d[bf], 0));
+            if (l >= 2) SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_d2h[bf], 0));
+            dq = sb; dk = sb + q_bytes; dv = sb + q_bytes + kv_bytes; dout = sb + q_bytes + 2 * kv_bytes;
+        }
+        if (staged) SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_load[bf], 0));
+        st = sc_prefill_layer_batched(pool, l, dq, dk, dv, tables_dev, max_blocks, n_seq, hist_lens, cu_new, bf,
+                                      mode, dout, xs);
+        if (st) return st;
+        if (staged) SC_CUDA(cudaEventRecord(pool->ev_attn[bf], xs));
+        if (host_io) {
+            SC_CUDA(cudaEventRecord(pool->ev_comp[bf], xs));
+            SC_CUDA(cudaStreamWaitEvent(pool->d2h_stream, pool->ev_comp[bf], 0));
+            SC_CUDA(cudaMemcpyAsync(o, dout, (size_t)q_bytes, cudaMemcpyDeviceToHost, pool->d2h_stream));
+            SC_CUDA(cudaEventRecord(pool->ev_d2h[bf], pool->d2h_stream));
+        }
+    }
+    if (host_io) {   // join: the compute stream finishes last
+        SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_d2h[(L - 1) & 1], 0));
+        if (L >= 2) SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_d2h[(L - 2) & 1], 0));
+    }
+    return SC_OK;
+}
+
+sc_status_t sc_launch_count(const sc_pool_t *pool, int64_t *n_launches)
+{
+    if (!pool || !n_launches) return sc_fail(SC_ERR_INVALID_ARG, "NULL argument");
+    *n_launches = pool->launches;
+    return SC_OK;
+}
+
+}  // extern "C"

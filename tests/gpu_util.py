@@ -1,0 +1,74 @@
+"""Shared helpers of the GPU parity tests: run the CUDA path through the C ABI and the
+CPU oracle on the same seeded inputs."""
+import numpy as np
+import torch
+
+from oracle import sc_oracle as O
+from paper_2606_16135_b200 import binding as sc
+from paper_2606_16135_b200 import inputs as I
+from paper_2606_16135_b200.runtime import Session, bits_to_torch, torch_to_bits
+
+MAX_ABS_TOL = 1e-2      # BASELINE.json north_star: bf16 output vs fp32 oracle
+REL_L2_TOL = 5e-3
+
+
+def errors(out_bits: np.ndarray, ref: np.ndarray):
+    got = I.bf16_bits_to_f32(out_bits).astype(np.float64)
+    ref = ref.astype(np.float64)
+    max_abs = float(np.abs(got - ref).max()) if ref.size else 0.0
+    rel = float(np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-30)) if ref.size else 0.0
+    return max_abs, rel
+
+
+def assert_close(out_bits, ref, what=""):
+    max_abs, rel = errors(out_bits, ref)
+    assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, f"{what}: max_abs={max_abs:.3e} rel_l2={rel:.3e}"
+    return max_abs, rel
+
+
+class Case:
+    """One conversation in one pool, mirrored in the oracle's pool."""
+
+    def __init__(self, L, Hq, Hkv, D, T_h, n, NB, seed, variant="normal", identity=False, perm_id=1,
+                 lsc_extra=2, split_tiles=0, max_new=None):
+        self.L, self.Hq, self.Hkv, self.D, self.T_h, self.n = L, Hq, Hkv, D, T_h, n
+        B = 16
+        nb_total = O.blocks_for(T_h + n, B)
+        assert NB >= nb_total
+        self.table = I.block_table(perm_id, NB, nb_total, identity=identity)
+        self.sess = Session(L, Hq, Hkv, D, B, NB, nb_total + lsc_extra, max_new or max(n, 1))
+        if split_tiles:
+            self.sess.pool.set_split_tiles(split_tiles)
+        self.opool = O.Pool(L, Hkv, D, B, NB)
+        self.table_dev = self.sess.table_dev(self.table)
+        self.data = []
+        for l in range(L):
+            q, kh, vh, kn, vn = I.make_qkv(n, T_h, Hq, Hkv, D, seed + 100 * l, variant)
+            self.data.append((q, kh, vh, kn, vn))
+            if T_h:
+                self.sess.store_prefix(l, bits_to_torch(kh, self.sess.device), bits_to_torch(vh, self.sess.device),
+                                       0, self.table_dev)
+                self.opool.store(l, 0, kh, 0, self.table)
+                self.opool.store(l, 1, vh, 0, self.table)
+        torch.cuda.synchronize()
+
+    def run_layer(self, l, mode, buf=0, load=True):
+        """CUDA path for layer l -> output bits [n][Hq][D]."""
+        s = self.sess
+        q, kh, vh, kn, vn = self.data[l]
+        dq, dk, dv = (bits_to_torch(x, s.device) for x in (q, kn, vn))
+        out = torch.zeros((self.n, self.Hq, self.D), dtype=torch.bfloat16, device=s.device)
+        st = torch.cuda.current_stream().cuda_stream
+        if mode == sc.SC_ATTN_STAGED and load:
+            s.pool.load_layer(l, self.table_dev.data_ptr(), len(self.table), self.T_h, buf, st)
+        s.pool.prefill_layer(l, dq.data_ptr(), dk.data_ptr(), dv.data_ptr(), self.table_dev.data_ptr(),
+                             len(self.table), self.T_h, self.n, buf, mode, out.data_ptr(), st)
+        torch.cuda.synchronize()
+        return torch_to_bits(out)
+
+    def oracle_layer(self, l):
+        q, kh, vh, kn, vn = self.data[l]
+        return O.prefill_layer(self.opool, l, q, kn, vn, self.table, self.T_h)
+
+    def close(self):
+        self.sess.close()

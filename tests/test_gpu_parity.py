@@ -1,0 +1,188 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the CPU oracle on the
+same seeded inputs.  KV movement and block-table indexing bit-exact; bf16 attention
+within max-abs 1e-2 and relative-L2 5e-3 of the fp32 oracle (BASELINE.json)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import sc_oracle as O
+from paper_2606_16135_b200 import binding as sc
+from paper_2606_16135_b200 import build as sc_build
+from paper_2606_16135_b200 import inputs as I
+from paper_2606_16135_b200.runtime import Session, bits_to_torch, torch_to_bits
+
+from gpu_util import Case, assert_close, errors
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built():
+    sc_build.build()
+    assert sc.lib() is not None
+
+
+MODES = [sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED]
+
+
+# ------------------------------------------------------------------ KV movement
+def test_store_prefix_places_every_element_where_the_accessor_says():
+    """a3 + the logical accessor: raw pool bytes at sc_cell_offset == the oracle's pool."""
+    c = Case(L=2, Hq=4, Hkv=4, D=64, T_h=509, n=0, NB=64, seed=3)
+    raw = c.sess.pool_mem.cpu().numpy().view(np.uint16)
+    rng = np.random.default_rng(0)
+    for l in range(2):
+        for kv in range(2):
+            want = c.opool.gather(l, kv, c.table, 509)
+            for _ in range(400):
+                t, h, d = int(rng.integers(509)), int(rng.integers(4)), int(rng.integers(64))
+                off = c.sess.pool.cell_offset(int(c.table[t // 16]), l, kv, h, t % 16, d)
+                assert raw[off // 2] == want[t, h, d]
+    # blocks outside the table were never touched (pool zero-filled at create)
+    other = np.setdiff1d(np.arange(64), c.table)
+    bb = c.sess.pool.info().block_bytes
+    for b in other[:8]:
+        assert not raw[b * bb // 2:(b + 1) * bb // 2].any()
+    c.close()
+
+
+@pytest.mark.parametrize("D,Hkv,T", [(64, 4, 509), (128, 2, 300), (128, 8, 16), (64, 1, 1)])
+def test_I1_store_then_read_is_bit_exact(D, Hkv, T):
+    c = Case(L=2, Hq=8, Hkv=Hkv, D=D, T_h=T, n=0, NB=40, seed=5)
+    for l in range(2):
+        k, v = c.sess.read_tokens(l, 0, c.table_dev, 0, T)
+        assert np.array_equal(torch_to_bits(k), c.data[l][1]) and np.array_equal(torch_to_bits(v), c.data[l][2])
+        assert np.array_equal(torch_to_bits(k), c.opool.gather(l, 0, c.table, T))
+        k2, v2 = c.sess.read_tokens(l, 0, c.table_dev, T // 2, T - T // 2)      # mid-block start
+        assert np.array_equal(torch_to_bits(v2), c.data[l][2][T // 2:])
+    c.close()
+
+
+@pytest.mark.parametrize("engine", [sc.SC_COPY_LDG, sc.SC_COPY_BULK])
+@pytest.mark.parametrize("D,Hkv,T", [(64, 4, 512), (128, 32, 200), (128, 8, 333), (64, 1, 17)])
+def test_I1_load_layer_gathers_history_bit_exact(engine, D, Hkv, T):
+    """a4: LSC[buf] holds the logically contiguous history after the paged gather."""
+    c = Case(L=2, Hq=32, Hkv=Hkv, D=D, T_h=T, n=0, NB=48, seed=7)
+    c.sess.pool.set_engine(sc.SC_ENGINE_AUTO, engine)
+    st = torch.cuda.current_stream().cuda_stream
+    for l, buf in ((0, 0), (1, 1), (0, 1)):
+        c.sess.pool.load_layer(l, c.table_dev.data_ptr(), len(c.table), T, buf, st)
+        k, v = c.sess.read_tokens(l, 1 + buf, None, 0, T)
+        assert np.array_equal(torch_to_bits(k), c.data[l][1]) and np.array_equal(torch_to_bits(v), c.data[l][2])
+    # whole-cell equality: LSC block j == pool cell (table[j], layer) byte for byte
+    info = c.sess.pool.info()
+    c.sess.pool.load_layer(1, c.table_dev.data_ptr(), len(c.table), T, 0, st)
+    torch.cuda.synchronize()
+    pool_raw, lsc_raw = c.sess.pool_mem.cpu().numpy(), c.sess.lsc_mem.cpu().numpy()
+    for j in range(O.blocks_for(T, 16)):
+        src = int(c.table[j]) * info.block_bytes + 1 * info.cell_bytes
+        assert np.array_equal(lsc_raw[j * info.cell_bytes:(j + 1) * info.cell_bytes],
+                              pool_raw[src:src + info.cell_bytes])
+    c.close()
+
+
+# ------------------------------------------------------------------ attention
+@pytest.mark.parametrize("mode", MODES)
+def test_tiny_config_matches_oracle(mode):
+    """BASELINE.json config 1: 2 layers, 4 heads, D 64, 512 history in a 64-block pool, 32 new."""
+    c = Case(L=2, Hq=4, Hkv=4, D=64, T_h=512, n=32, NB=64, seed=16135)
+    for l in range(2):
+        got = c.run_layer(l, mode, buf=l & 1)
+        assert_close(got, c.oracle_layer(l), f"layer {l}")
+        # I2: the turn's K/V were scattered back: pool now holds [history ; new] bit-exactly
+        k, v = c.sess.read_tokens(l, 0, c.table_dev, 0, 544)
+        assert np.array_equal(torch_to_bits(k), c.opool.gather(l, 0, c.table, 544))
+        assert np.array_equal(torch_to_bits(v), np.concatenate([c.data[l][2], c.data[l][4]]))
+        if mode == sc.SC_ATTN_STAGED:
+            k, v = c.sess.read_tokens(l, 1 + (l & 1), None, 0, 544)
+            assert np.array_equal(torch_to_bits(k), np.concatenate([c.data[l][1], c.data[l][3]]))
+    c.close()
+
+
+@pytest.mark.parametrize("T_h", [0, 1, 15, 16, 17, 509])
+@pytest.mark.parametrize("n", [1, 31, 32, 33, 256])
+def test_edge_lengths(T_h, n):
+    mode = MODES[(T_h + n) % 2]
+    c = Case(L=1, Hq=4, Hkv=4, D=64, T_h=T_h, n=n, NB=64, seed=1000 + T_h * 7 + n)
+    assert_close(c.run_layer(0, mode), c.oracle_layer(0), f"T_h={T_h} n={n}")
+    k, v = c.sess.read_tokens(0, 0, c.table_dev, 0, T_h + n)
+    assert np.array_equal(torch_to_bits(k), c.opool.gather(0, 0, c.table, T_h + n))
+    c.close()
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("variant", ["normal", "peaked", "adversarial"])
+@pytest.mark.parametrize("Hq,Hkv,D", [(8, 2, 128), (4, 4, 128), (8, 8, 64), (4, 1, 64)])
+def test_shapes_and_score_distributions(mode, variant, Hq, Hkv, D):
+    """GQA 4:1, MHA, D 64/128; peaked and adversarial scores force the running-max rescale."""
+    c = Case(L=1, Hq=Hq, Hkv=Hkv, D=D, T_h=700, n=70, NB=64, seed=77, variant=variant)
+    assert_close(c.run_layer(0, mode), c.oracle_layer(0), f"{variant} {Hq}/{Hkv}/{D}")
+    c.close()
+
+
+@pytest.mark.parametrize("split_tiles", [1, 2, 3, 5, 1000])
+def test_split_kv_and_combine(split_tiles):
+    """a7: any partition of the keys gives the same answer within tolerance, including
+    partitions whose last split is fully masked for the first rows."""
+    c = Case(L=1, Hq=4, Hkv=2, D=128, T_h=777, n=200, NB=80, seed=91, variant="peaked",
+             split_tiles=split_tiles)
+    ref = c.oracle_layer(0)
+    assert_close(c.run_layer(0, sc.SC_ATTN_FUSED), ref, f"split_tiles={split_tiles}")
+    c.close()
+
+
+def test_I5_block_permutation_gives_bit_identical_output():
+    """I5 on the GPU: work partitioning depends on logical positions only."""
+    outs = []
+    for perm_id, ident in ((1, False), (2, False), (1, True)):
+        c = Case(L=1, Hq=8, Hkv=2, D=128, T_h=1000, n=100, NB=96, seed=55, perm_id=perm_id, identity=ident)
+        outs.append((c.run_layer(0, sc.SC_ATTN_FUSED), c.run_layer(0, sc.SC_ATTN_STAGED)))
+        c.close()
+    for fused, staged in outs[1:]:
+        assert np.array_equal(fused, outs[0][0]) and np.array_equal(staged, outs[0][1])
+    assert np.array_equal(outs[0][0], outs[0][1])          # same kernel, identity table over the LSC
+
+
+def test_softmax_invariants_on_gpu():
+    """I4 through the CUDA path: V == 1 gives exactly 1.0; q == 0 gives the running mean of V."""
+    c = Case(L=1, Hq=4, Hkv=2, D=64, T_h=300, n=40, NB=32, seed=66)
+    q, kh, vh, kn, vn = c.data[0]
+    ones = np.full_like(vh, 0x3F80)
+    c.sess.store_prefix(0, bits_to_torch(kh, c.sess.device), bits_to_torch(ones, c.sess.device), 0, c.table_dev)
+    c.data[0] = (q, kh, ones, kn, np.full_like(vn, 0x3F80))
+    got = I.bf16_bits_to_f32(c.run_layer(0, sc.SC_ATTN_FUSED))
+    assert np.abs(got - 1).max() <= 2 ** -8
+    c.close()
+    c = Case(L=1, Hq=4, Hkv=2, D=64, T_h=45, n=9, NB=8, seed=67)
+    q, kh, vh, kn, vn = c.data[0]
+    c.data[0] = (np.zeros_like(q), kh, vh, kn, vn)
+    got = I.bf16_bits_to_f32(c.run_layer(0, sc.SC_ATTN_STAGED))
+    V = I.bf16_bits_to_f32(np.concatenate([vh, vn])).astype(np.float64)
+    for i in range(9):
+        want = V[:45 + i + 1].mean(axis=0)
+        for h in range(4):
+            assert np.abs(got[i, h] - want[h // 2]).max() < 4e-3
+    c.close()
+
+
+# ------------------------------------------------------------------ errors
+def test_argument_errors_launch_nothing():
+    c = Case(L=1, Hq=4, Hkv=4, D=64, T_h=64, n=16, NB=16, seed=1)
+    p, t = c.sess.pool, c.table_dev
+    before = p.launch_count()
+    x = torch.zeros(16 * 4 * 64, dtype=torch.bfloat16, device=c.sess.device).data_ptr()
+    bad = [
+        (sc.SC_ERR_INVALID_ARG, lambda: p.prefill_layer(1, x, x, x, t.data_ptr(), len(c.table), 64, 16, 0, 1, x)),
+        (sc.SC_ERR_CAPACITY, lambda: p.prefill_layer(0, x, x, x, t.data_ptr(), 4, 64, 16, 0, 1, x)),
+        (sc.SC_ERR_CAPACITY, lambda: p.prefill_layer(0, x, x, x, t.data_ptr(), len(c.table), 64, 17, 0, 1, x)),
+        (sc.SC_ERR_INVALID_ARG, lambda: p.prefill_layer(0, 0, x, x, t.data_ptr(), len(c.table), 64, 16, 0, 1, x)),
+        (sc.SC_ERR_INVALID_ARG, lambda: p.prefill_layer(0, x, x, x, t.data_ptr(), len(c.table), 64, 16, 2, 0, x)),
+        (sc.SC_ERR_CAPACITY, lambda: p.load_layer(0, t.data_ptr(), 2, 64, 0)),
+        (sc.SC_ERR_CAPACITY, lambda: p.store_prefix(0, x, x, 0, 16 * 6, t.data_ptr(), len(c.table))),
+    ]
+    for status, call in bad:
+        with pytest.raises(sc.SwiftCacheError) as e:
+            call()
+        assert e.value.status == status, str(e.value)
+    assert p.launch_count() == before
+    c.close()

@@ -1,0 +1,191 @@
+"""GPU parity of the ragged batch (a9), the multi-turn loop (O6) and the layer-streaming
+pipeline (a8), all through the C ABI against the CPU oracle."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import sc_oracle as O
+from paper_2606_16135_b200 import binding as sc
+from paper_2606_16135_b200 import build as sc_build
+from paper_2606_16135_b200 import inputs as I
+from paper_2606_16135_b200.runtime import Session, bits_to_torch, torch_to_bits
+
+from gpu_util import assert_close
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built():
+    sc_build.build()
+
+
+class Conversations:
+    """n_seq conversations sharing one pool; tables come from the library's allocator and are
+    mirrored, id for id, in the oracle's pool."""
+
+    def __init__(self, L, Hq, Hkv, D, hist, NB, max_new, seed, pool_kind=sc.SC_POOL_HBM, lsc_blocks=None):
+        self.L, self.Hq, self.Hkv, self.D, self.B = L, Hq, Hkv, D, 16
+        self.n_seq = len(hist)
+        self.hist = list(hist)
+        self.max_blocks = max(O.blocks_for(h, 16) for h in hist) + 64
+        if lsc_blocks is None:
+            lsc_blocks = sum(O.blocks_for(h, 16) for h in hist) + 64 * self.n_seq
+        self.sess = Session(L, Hq, Hkv, D, 16, NB, lsc_blocks, max_new, max_seqs=self.n_seq,
+                            pool_kind=pool_kind, alloc_seed=seed)
+        self.opool = O.Pool(L, Hkv, D, 16, NB)
+        self.tables = np.full((self.n_seq, self.max_blocks), -1, dtype=np.int32)
+        self.n_table = [0] * self.n_seq
+        self.logical = [[[None, None] for _ in range(L)] for _ in range(self.n_seq)]
+        dev = self.sess.device
+        for s, h in enumerate(hist):
+            self.n_table[s] = self.sess.pool.append_blocks(self.tables[s], 0, 0, h)
+        self.tables_dev = self.sess.table_dev(self.tables)
+        for s, h in enumerate(hist):
+            for l in range(L):
+                kh = I.normal_bf16((h, Hkv, D), seed + 1000 * s + 10 * l)
+                vh = I.normal_bf16((h, Hkv, D), seed + 1000 * s + 10 * l + 5)
+                self.logical[s][l] = [kh, vh]
+                if h:
+                    self.sess.store_prefix(l, bits_to_torch(kh, dev), bits_to_torch(vh, dev), 0,
+                                           self.tables_dev[s])
+                    self.opool.store(l, 0, kh, 0, self.tables[s][:self.n_table[s]])
+                    self.opool.store(l, 1, vh, 0, self.tables[s][:self.n_table[s]])
+        torch.cuda.synchronize()
+
+    def begin_turn(self, n_new):
+        for s in range(self.n_seq):
+            self.n_table[s] = self.sess.pool.append_blocks(self.tables[s], self.n_table[s], self.hist[s], n_new[s])
+        self.tables_dev.copy_(torch.from_numpy(self.tables))
+        all_ids = np.concatenate([self.tables[s][:self.n_table[s]] for s in range(self.n_seq)])
+        assert len(set(all_ids.tolist())) == len(all_ids)            # tables stay pairwise disjoint
+        self.cu = np.concatenate([[0], np.cumsum(n_new)]).astype(np.int32)
+
+    def make_inputs(self, n_new, seed, variant="normal"):
+        """q/k/v for every layer, packed over the batch: bits [L][sum n][H][D]."""
+        qs, ks, vs = [], [], []
+        for l in range(self.L):
+            ql, kl, vl = [], [], []
+            for s in range(self.n_seq):
+                q, _, _, kn, vn = I.make_qkv(n_new[s], 0, self.Hq, self.Hkv, self.D, seed + 97 * l + 13 * s, variant)
+                ql.append(q); kl.append(kn); vl.append(vn)
+            qs.append(np.concatenate(ql)); ks.append(np.concatenate(kl)); vs.append(np.concatenate(vl))
+        return np.stack(qs), np.stack(ks), np.stack(vs)
+
+    def oracle_turn(self, q_all, k_all, v_all):
+        outs = []
+        for l in range(self.L):
+            rows = []
+            for s in range(self.n_seq):
+                a, b = self.cu[s], self.cu[s + 1]
+                tab = self.tables[s][:self.n_table[s]]
+                rows.append(O.prefill_layer(self.opool, l, q_all[l][a:b], k_all[l][a:b], v_all[l][a:b], tab, self.hist[s]))
+                self.logical[s][l][0] = np.concatenate([self.logical[s][l][0], k_all[l][a:b]])
+                self.logical[s][l][1] = np.concatenate([self.logical[s][l][1], v_all[l][a:b]])
+            outs.append(np.concatenate(rows))
+        return np.stack(outs)
+
+    def end_turn(self, n_new):
+        for s in range(self.n_seq):
+            self.hist[s] += int(n_new[s])
+
+    def check_pool_equals_logical(self):
+        for s in range(self.n_seq):
+            for l in range(self.L):
+                k, v = self.sess.read_tokens(l, 0, self.tables_dev[s], 0, self.hist[s])
+                assert np.array_equal(torch_to_bits(k), self.logical[s][l][0])
+                assert np.array_equal(torch_to_bits(v), self.logical[s][l][1])
+
+
+@pytest.mark.parametrize("mode", [sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED])
+def test_ragged_batch_multi_turn(mode):
+    """Config 5 in miniature: ragged histories (remainders mod 16: 5, 12, 0, 1), ragged n_new,
+    3 turns; every turn's new KV is scattered back and read by the next turn (I2, O6)."""
+    cv = Conversations(L=2, Hq=4, Hkv=2, D=64, hist=[37, 300, 16, 1025], NB=220, max_new=200, seed=5)
+    p, dev = cv.sess.pool, cv.sess.device
+    st = torch.cuda.current_stream().cuda_stream
+    for turn in range(3):
+        n_new = [20 + turn, 33, 16, 64 - turn]
+        cv.begin_turn(n_new)
+        q_all, k_all, v_all = cv.make_inputs(n_new, 900 + turn)
+        ref = cv.oracle_turn(q_all, k_all, v_all)
+        for l in range(cv.L):
+            dq, dk, dv = (bits_to_torch(x[l], dev) for x in (q_all, k_all, v_all))
+            out = torch.zeros_like(dq)
+            if mode == sc.SC_ATTN_STAGED:
+                p.load_layer_batched(l, cv.tables_dev.data_ptr(), cv.max_blocks, cv.hist, cv.cu, l & 1, st)
+            p.prefill_layer_batched(l, dq.data_ptr(), dk.data_ptr(), dv.data_ptr(), cv.tables_dev.data_ptr(),
+                                    cv.max_blocks, cv.hist, cv.cu, l & 1, mode, out.data_ptr(), st)
+            torch.cuda.synchronize()
+            assert_close(torch_to_bits(out), ref[l], f"turn {turn} layer {l}")
+        cv.end_turn(n_new)
+        cv.check_pool_equals_logical()
+    cv.sess.close()
+
+
+@pytest.mark.parametrize("io_kind", [sc.SC_MEM_DEVICE, sc.SC_MEM_HOST_PINNED])
+@pytest.mark.parametrize("mode", [sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED])
+def test_prefill_turn_pipeline(mode, io_kind):
+    """a8: the two-stream, double-buffered pipeline over L layers, several turns issued back
+    to back with no host synchronisation in between (PAPER.md:192 ordering rule)."""
+    cv = Conversations(L=5, Hq=8, Hkv=2, D=128, hist=[700, 45], NB=200, max_new=160, seed=9)
+    p, dev = cv.sess.pool, cv.sess.device
+    refs, outs, keep = [], [], []
+    for turn in range(3):
+        n_new = [96, 40 + turn]
+        cv.begin_turn(n_new)
+        q_all, k_all, v_all = cv.make_inputs(n_new, 300 + turn, "peaked" if turn == 1 else "normal")
+        refs.append(cv.oracle_turn(q_all, k_all, v_all))
+        if io_kind == sc.SC_MEM_HOST_PINNED:
+            tq, tk, tv = (bits_to_torch(x).pin_memory() for x in (q_all, k_all, v_all))
+            out = torch.zeros(tq.shape, dtype=torch.bfloat16).pin_memory()
+        else:
+            tq, tk, tv = (bits_to_torch(x, dev) for x in (q_all, k_all, v_all))
+            out = torch.zeros_like(tq)
+            torch.cuda.synchronize()
+        keep.append((tq, tk, tv))
+        cv.sess.compute_stream.wait_stream(torch.cuda.current_stream())   # table upload, inputs
+        p.prefill_turn(tq.data_ptr(), tk.data_ptr(), tv.data_ptr(), out.data_ptr(), io_kind,
+                       cv.tables_dev.data_ptr(), cv.max_blocks, cv.hist, cv.cu, mode,
+                       cv.sess.copy_stream.cuda_stream, cv.sess.compute_stream.cuda_stream)
+        outs.append(out)
+        cv.end_turn(n_new)
+        # tables_dev is rewritten by the next begin_turn on the current stream: order it
+        torch.cuda.current_stream().wait_stream(cv.sess.compute_stream)
+    torch.cuda.synchronize()
+    for turn in range(3):
+        for l in range(cv.L):
+            assert_close(torch_to_bits(outs[turn][l]), refs[turn][l], f"turn {turn} layer {l}")
+    cv.check_pool_equals_logical()
+    cv.sess.close()
+
+
+def test_host_pinned_pool_matches_oracle():
+    """Config 4's second variant in miniature: the pool lives in pinned host memory (the PCIe
+    reload path); gather, scatter and fused attention read and write it directly."""
+    cv = Conversations(L=2, Hq=8, Hkv=2, D=128, hist=[333], NB=40, max_new=64, seed=21,
+                       pool_kind=sc.SC_POOL_HOST_PINNED)
+    p, dev = cv.sess.pool, cv.sess.device
+    st = torch.cuda.current_stream().cuda_stream
+    for turn, mode in enumerate([sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED]):
+        n_new = [50]
+        cv.begin_turn(n_new)
+        q_all, k_all, v_all = cv.make_inputs(n_new, 40 + turn)
+        ref = cv.oracle_turn(q_all, k_all, v_all)
+        for l in range(cv.L):
+            dq, dk, dv = (bits_to_torch(x[l], dev) for x in (q_all, k_all, v_all))
+            out = torch.zeros_like(dq)
+            if mode == sc.SC_ATTN_STAGED:
+                p.load_layer_batched(l, cv.tables_dev.data_ptr(), cv.max_blocks, cv.hist, cv.cu, 0, st)
+            p.prefill_layer_batched(l, dq.data_ptr(), dk.data_ptr(), dv.data_ptr(), cv.tables_dev.data_ptr(),
+                                    cv.max_blocks, cv.hist, cv.cu, 0, mode, out.data_ptr(), st)
+            torch.cuda.synchronize()
+            assert_close(torch_to_bits(out), ref[l], f"host pool turn {turn} layer {l}")
+        cv.end_turn(n_new)
+        cv.check_pool_equals_logical()
+    # the host copy itself holds the bytes (the CPU can see what the GPU scattered)
+    raw = cv.sess.pool_mem.numpy().view(np.uint16)
+    t, h, d = 370, 1, 77
+    off = p.cell_offset(int(cv.tables[0][t // 16]), 1, 0, h, t % 16, d)
+    assert raw[off // 2] == cv.logical[0][1][0][t, h, d]
+    cv.sess.close()
