@@ -1,0 +1,465 @@
+#!/usr/bin/env python
+"""bench.py -- per-turn layer-streamed prefill on one B200 (BASELINE.json metric).
+
+A "step" is one whole turn of the hot path (all SURVEY.md 8(a) rows) over one batch of
+synthetic input: for each of the L layers, paged gather of the history KV pool -> LSC on the
+copy stream, scatter of the turn's new K/V into pool blocks, causal attention of the new
+tokens over history + themselves, split-KV combine; two streams, double-buffered LSC.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload lwm_5k] [--mode staged|fused]
+    python bench.py --impl reference ...     # the CPU oracle, as it stands, on the host cores
+
+Prints ONE JSON line (rank 0).  See DESIGN.md section 7 for what every key means.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "per-turn layer-streamed prefill ms (256 new tok) & paged-KV GB/s vs HBM peak"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="lwm_5k")
+    ap.add_argument("--mode", default="staged", choices=["staged", "fused"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "mma", "tcgen05"])
+    ap.add_argument("--copy", default="auto", choices=["auto", "ldg", "bulk"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        p["_source"] = "measured"
+        return p
+    p = dict(FALLBACK_PEAKS)
+    p["_source"] = "fallback"
+    return p
+
+
+# ------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------- workload
+def flops_per_layer(shape, hist, n):
+    """4*Hq*D*n*(T_h + (n+1)/2): QK^T and PV, 2 flop per MAC, causal triangle counted once."""
+    return 4.0 * shape.Hq * shape.D * n * (hist + (n + 1) / 2.0)
+
+
+class Workload:
+    """Synthetic conversations of one BASELINE.json config, resident in HBM."""
+
+    def __init__(self, name: str, device, engine="auto", copy="auto", keep_host_layers=1):
+        import torch
+        from paper_2606_16135_b200 import binding as sc
+        from paper_2606_16135_b200 import inputs as I
+        from paper_2606_16135_b200.runtime import Session
+
+        self.torch, self.sc, self.I = torch, sc, I
+        shape = I.configs()[name]
+        self.shape, self.name = shape, name
+        B = shape.B
+        self.n_seq = len(shape.hist)
+        self.hist = list(shape.hist)
+        self.n_new = [shape.n_new] * self.n_seq
+        self.cu = np.concatenate([[0], np.cumsum(self.n_new)]).astype(np.int32)
+        blocks = [-(-(h + n) // B) for h, n in zip(self.hist, self.n_new)]
+        self.max_blocks = max(blocks)
+        pool_kind = sc.SC_POOL_HOST_PINNED if shape.pool_kind == "host" else sc.SC_POOL_HBM
+        self.sess = Session(shape.L, shape.Hq, shape.Hkv, shape.D, B, shape.n_blocks, sum(blocks),
+                            int(self.cu[-1]), max_seqs=self.n_seq, pool_kind=pool_kind,
+                            alloc_seed=I.BASE_SEED + shape.config_id, device=device)
+        eng = {"auto": sc.SC_ENGINE_AUTO, "mma": sc.SC_ENGINE_MMA_SYNC, "tcgen05": sc.SC_ENGINE_TCGEN05}[engine]
+        cpy = {"auto": sc.SC_COPY_AUTO, "ldg": sc.SC_COPY_LDG, "bulk": sc.SC_COPY_BULK}[copy]
+        self.sess.pool.set_engine(eng, cpy)
+        # tables: the library's allocator hands out a seeded shuffle of the pool ("shuffled pool")
+        self.tables = np.full((self.n_seq, self.max_blocks), -1, dtype=np.int32)
+        self.n_table = []
+        for s in range(self.n_seq):
+            nt = self.sess.pool.append_blocks(self.tables[s], 0, 0, self.hist[s])
+            nt = self.sess.pool.append_blocks(self.tables[s], nt, self.hist[s], self.n_new[s])
+            self.n_table.append(nt)
+        self.tables_dev = self.sess.table_dev(self.tables)
+        # history: one layer at a time, generated on the device from its seed, stored via the ABI
+        self.host_hist = {}
+        dev = self.sess.device
+        for l in range(shape.L):
+            for s in range(self.n_seq):
+                k = I.normal_bf16_device((self.hist[s], shape.Hkv, shape.D), I.seed_for(shape.config_id, l, "k", conv=s), dev)
+                v = I.normal_bf16_device((self.hist[s], shape.Hkv, shape.D), I.seed_for(shape.config_id, l, "v", conv=s), dev)
+                self.sess.store_prefix(l, k, v, 0, self.tables_dev[s])
+                if l < keep_host_layers:
+                    self.host_hist[(l, s)] = (k.view(torch.int16).cpu().numpy().view(np.uint16),
+                                              v.view(torch.int16).cpu().numpy().view(np.uint16))
+            torch.cuda.synchronize()
+        tot = int(self.cu[-1])
+        self.q = I.normal_bf16_device((shape.L, tot, shape.Hq, shape.D), I.seed_for(shape.config_id, 0, "q"), dev)
+        self.k = I.normal_bf16_device((shape.L, tot, shape.Hkv, shape.D), I.seed_for(shape.config_id, 0, "k_new"), dev)
+        self.v = I.normal_bf16_device((shape.L, tot, shape.Hkv, shape.D), I.seed_for(shape.config_id, 0, "v_new"), dev)
+        self.out = torch.zeros_like(self.q)
+        torch.cuda.synchronize()
+
+    def turn(self, mode, io="device", bufs=None):
+        sc, s = self.sc, self.sess
+        q, k, v, out = bufs if bufs is not None else (self.q, self.k, self.v, self.out)
+        s.pool.prefill_turn(q.data_ptr(), k.data_ptr(), v.data_ptr(), out.data_ptr(),
+                            sc.SC_MEM_HOST_PINNED if io == "host" else sc.SC_MEM_DEVICE,
+                            self.tables_dev.data_ptr(), self.max_blocks, self.hist, self.cu, mode,
+                            s.copy_stream.cuda_stream, s.compute_stream.cuda_stream)
+
+    # algorithmic work of one layer
+    def layer_flops(self):
+        return sum(flops_per_layer(self.shape, h, n) for h, n in zip(self.hist, self.n_new))
+
+    def layer_gather_bytes(self):
+        cell = self.sess.pool.info().cell_bytes
+        return 2.0 * sum(-(-h // self.shape.B) for h in self.hist) * cell      # read + write
+
+    def layer_hist_kv_bytes(self):
+        return float(sum(self.hist)) * self.shape.tok_bytes
+
+    def layer_scatter_bytes(self, staged):
+        return float(self.cu[-1]) * self.shape.tok_bytes * (3.0 if staged else 2.0)
+
+
+# ------------------------------------------------------------------ CPU baseline
+def oracle_sample(w: "Workload", rows=32, budget_s=12.0, max_steps=None):
+    """Times the CPU oracle, as it stands, on a bounded sample of the same workload: layer 0
+    of conversation 0, the whole layer's paged gather + scatter and the attention of `rows`
+    middle new-token rows over the full history, repeated until `budget_s` is spent.
+    Returns (ms per turn extrapolated to L layers x n rows x all conversations, info)."""
+    from oracle import sc_oracle as O
+    I, shape = w.I, w.shape
+    n, T_h = w.n_new[0], w.hist[0]
+    kh, vh = w.host_hist[(0, 0)]
+    tab = w.tables[0][:w.n_table[0]]
+    # the oracle's own pool, one layer deep, same block ids
+    opool = O.Pool(1, shape.Hkv, shape.D, shape.B, shape.n_blocks)
+    opool.store(0, 0, kh, 0, tab)
+    opool.store(0, 1, vh, 0, tab)
+    torch = w.torch
+    q = w.q[0, :n].view(torch.int16).cpu().numpy().view(np.uint16)
+    kn = w.k[0, :n].view(torch.int16).cpu().numpy().view(np.uint16)
+    vn = w.v[0, :n].view(torch.int16).cpu().numpy().view(np.uint16)
+    a = max(0, n // 2 - rows // 2)
+    b = min(n, a + rows)
+    t_move, t_attn, steps, out = [], [], 0, None
+    t_start = time.perf_counter()
+    while True:
+        t0 = time.perf_counter()
+        lk = opool.gather(0, 0, tab, T_h)
+        lv = opool.gather(0, 1, tab, T_h)
+        opool.store(0, 0, kn, T_h, tab)
+        opool.store(0, 1, vn, T_h, tab)
+        t1 = time.perf_counter()
+        K = np.concatenate([lk, kn[:b]])
+        V = np.concatenate([lv, vn[:b]])
+        out = O.attention(q[a:b], K, V, T_h + a)
+        t2 = time.perf_counter()
+        t_move.append(t1 - t0)
+        t_attn.append(t2 - t1)
+        steps += 1
+        if (max_steps and steps >= max_steps) or (not max_steps and time.perf_counter() - t_start > budget_s):
+            break
+    scale_rows = n / float(b - a)
+    work_ratio = sum(flops_per_layer(shape, h, m) for h, m in zip(w.hist, w.n_new)) / flops_per_layer(shape, T_h, n)
+    move_ratio = sum(w.hist) / float(T_h)
+    per_layer_s = np.mean(t_move) * move_ratio + np.mean(t_attn) * scale_rows * work_ratio
+    info = {"cores": O.openmp_threads(), "kind": "oracle",
+            "sample": (f"layer 0, conversation 0: full-layer paged gather+scatter ({np.mean(t_move)*1e3:.0f} ms) + "
+                       f"attention of new-token rows [{a},{b}) x {shape.Hq} heads over {T_h}+{n} keys "
+                       f"({np.mean(t_attn)*1e3:.0f} ms), {steps} repeats; extrapolated x{scale_rows:.0f} rows "
+                       f"x{shape.L} layers" + (f" x{work_ratio:.2f} conversations" if w.n_seq > 1 else "")),
+            "step_s": [float(x + y) for x, y in zip(t_move, t_attn)]}
+    return per_layer_s * shape.L * 1e3, info, (a, b, out)
+
+
+# ------------------------------------------------------------------------- ours
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_16135_b200 import build as sc_build
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    if rank == 0:
+        sc_build.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        dist.barrier()
+    device = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(device)
+    from paper_2606_16135_b200 import binding as sc
+
+    w = Workload(args.workload, device, args.engine, args.copy)
+    shape, pool, xs = w.shape, w.sess.pool, w.sess.compute_stream
+    mode = sc.SC_ATTN_STAGED if args.mode == "staged" else sc.SC_ATTN_FUSED
+    pk = peaks()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed(n_steps, io="device", bufs=None):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        ev0.record(xs)
+        for _ in range(n_steps):
+            w.turn(mode, io, bufs)
+        ev1.record(xs)
+        barrier()
+        ms = ev0.elapsed_time(ev1)
+        if world > 1:
+            t = torch.tensor([ms], device=device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    # warm-up, then the timed region (inputs resident in HBM)
+    for _ in range(max(args.warmup, 3)):
+        w.turn(mode)
+    barrier()
+    clk = ClockSampler(local) if rank == 0 else None
+    l0 = pool.launch_count()
+    total_ms = timed(args.steps)
+    launches = pool.launch_count() - l0
+    clocks = clk.stop() if clk else None
+    ms_per_step = total_ms / args.steps
+
+    # end to end through the C ABI with HOST buffers (pinned): H2D of q/k/v and D2H of out inside
+    e2e = None
+    if not args.no_e2e:
+        hq, hk, hv = (t.cpu().pin_memory() for t in (w.q, w.k, w.v))
+        hout = torch.zeros(w.q.shape, dtype=torch.bfloat16).pin_memory()
+        bufs = (hq, hk, hv, hout)
+        for _ in range(3):
+            w.turn(mode, "host", bufs)
+        e_steps = max(3, min(args.steps, 20))
+        e_ms = timed(e_steps, "host", bufs) / e_steps
+        h2d = sum(int(t.numel()) * 2 for t in (hq, hk, hv))
+        d2h = int(hout.numel()) * 2
+        e2e = {"value": round(e_ms, 4), "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "pcie_gbs": round((h2d + d2h) / e_ms / 1e6, 2)}
+
+    # per-kernel device times: events around every launch, on its own stream, inside the pipeline
+    pool.profile_enable(True)
+    p_steps = 5
+    for _ in range(p_steps):
+        w.turn(mode)
+    torch.cuda.synchronize()
+    prof = pool.profile_collect()
+    pool.profile_enable(False)
+    # and each kernel alone (no concurrent stream): gather over all layers, fused attention
+    iso = {}
+    st = xs.cuda_stream
+    pool.profile_enable(True)
+    for _ in range(3):
+        for l in range(shape.L):
+            pool.load_layer_batched(l, w.tables_dev.data_ptr(), w.max_blocks, w.hist, w.cu, l & 1, st)
+    torch.cuda.synchronize()
+    iso["gather"] = pool.profile_collect()["gather"]
+    pool.profile_enable(True)
+    for _ in range(3):
+        for l in range(shape.L):
+            pool.prefill_layer_batched(l, w.q[l].data_ptr(), w.k[l].data_ptr(), w.v[l].data_ptr(),
+                                       w.tables_dev.data_ptr(), w.max_blocks, w.hist, w.cu, 0,
+                                       sc.SC_ATTN_FUSED, w.out[l].data_ptr(), st)
+    torch.cuda.synchronize()
+    c = pool.profile_collect()
+    iso["attention_fused"], iso["scatter"], iso["combine"] = c["attention"], c["scatter"], c["combine"]
+    pool.profile_enable(False)
+
+    def avg(rec):
+        return rec[0] / rec[1] if rec[1] else None
+
+    staged = mode == sc.SC_ATTN_STAGED
+    work = {"gather": ("hbm", w.layer_gather_bytes()), "attention": ("tensor", w.layer_flops()),
+            "scatter": ("hbm", w.layer_scatter_bytes(staged)), "combine": ("hbm", None)}
+    kernels = {}
+    for name, rec in prof.items():
+        a = avg(rec)
+        if a is None:
+            continue
+        bound, amount = work[name]
+        k = {"avg_ms": round(a, 5), "launches_per_turn": rec[1] // p_steps, "share": None, "bound": bound}
+        if amount:
+            if bound == "hbm":
+                k["achieved_GBs"] = round(amount / a / 1e6, 1)
+                k["frac_of_measured_hbm"] = round(amount / a / 1e6 / pk["hbm_gbs"], 4)
+            else:
+                k["achieved_TFLOPs"] = round(amount / a / 1e9, 1)
+                k["frac_of_measured_bf16_sustained"] = round(amount / a / 1e9 / pk["bf16_tflops_sustained"], 4)
+        kernels[name] = k
+    tot = sum(rec[0] for rec in prof.values())
+    for name, rec in prof.items():
+        if name in kernels:
+            kernels[name]["share"] = round(rec[0] / tot, 4)
+    dom = max(prof, key=lambda n: prof[n][0])
+    d_avg = avg(prof[dom])
+    bound, amount = work[dom]
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(f"{args.workload}:{dom}")
+    if bound == "hbm":
+        roof = {"kernel": dom, "bound": "hbm", "achieved": round(amount / d_avg / 1e6, 1), "peak": pk["hbm_gbs"],
+                "unit": "GB/s", "peak_source": pk["_source"] + " copy bandwidth"}
+    else:
+        roof = {"kernel": dom, "bound": "tensor", "achieved": round(amount / d_avg / 1e9, 1),
+                "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                "peak_source": pk["_source"] + " cuBLAS bf16, sustained (kernel timed inside a long step)"}
+    roof["frac"] = round(roof["achieved"] / roof["peak"], 4)
+    roof["traffic"] = traffic
+    roof["avg_launch_ms"] = round(d_avg, 5)
+
+    # the oracle beside it (rank 0, bounded sample) and a parity spot check on that sample
+    cpu, parity = None, None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu_ms, info, (a, b, ref) = oracle_sample(w)
+        got = w.I.bf16_bits_to_f32(w.out[0, a:b].view(torch.int16).cpu().numpy().view(np.uint16)).astype(np.float64)
+        parity = {"layer": 0, "rows": [a, b], "max_abs": float(np.abs(got - ref).max()),
+                  "rel_l2": float(np.linalg.norm(got - ref) / np.linalg.norm(ref)), "tol": [1e-2, 5e-3]}
+        info.pop("step_s")
+        cpu = {"value": round(cpu_ms, 1), "unit": "ms", **info}
+
+    kv_turn_bytes = w.layer_hist_kv_bytes() * shape.L
+    line = {
+        "metric": METRIC, "value": round(ms_per_step, 4), "unit": "ms", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: {shape.L} layers, {shape.Hq}q/{shape.Hkv}kv heads, D {shape.D}, "
+                               f"block {shape.B}, history {list(w.hist)} tokens in a shuffled {shape.n_blocks}-block "
+                               f"{'pinned-host' if shape.pool_kind == 'host' else 'HBM'} pool, {shape.n_new} new tokens",
+                   "mode": args.mode, "replicas": world,
+                   "l2": f"inputs larger than L2: each turn streams {kv_turn_bytes/1e9:.2f} GB of pool KV"},
+        "kv_gbs": round(world * kv_turn_bytes / ms_per_step / 1e6, 1),
+        "attn_tflops": round(world * w.layer_flops() * shape.L / ms_per_step / 1e9, 1),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        "roofline": roof, "kernels": kernels,
+        "isolated": {k: {"avg_ms": round(avg(v), 5)} for k, v in iso.items() if avg(v) is not None},
+        "cpu_baseline": cpu, "parity": parity,
+    }
+    g = avg(iso["gather"])
+    if g:
+        line["isolated"]["gather"]["GBs"] = round(w.layer_gather_bytes() / g / 1e6, 1)
+        line["isolated"]["gather"]["frac_of_measured_hbm"] = round(w.layer_gather_bytes() / g / 1e6 / pk["hbm_gbs"], 4)
+    af = avg(iso["attention_fused"])
+    if af:
+        line["isolated"]["attention_fused"]["TFLOPs"] = round(w.layer_flops() / af / 1e9, 1)
+        line["isolated"]["attention_fused"]["kv_read_GBs"] = round(w.layer_hist_kv_bytes() / af / 1e6, 1)
+    if rank == 0:
+        print(json.dumps(line))
+    w.sess.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# -------------------------------------------------------------------- reference
+def run_reference(args):
+    """The CPU oracle, as it stands, on the host cores: same config, metric and unit.  Each
+    step is a bounded sample of the workload (see oracle_sample); rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import torch
+    if not torch.cuda.is_available():
+        print(json.dumps({"impl": "reference", "unavailable": "inputs are generated on the CUDA device"}))
+        return
+    from paper_2606_16135_b200 import build as sc_build
+    sc_build.build()
+    w = Workload(args.workload, torch.device("cuda:0"))
+    shape = w.shape
+    oracle_sample(w, max_steps=max(args.warmup, 1))
+    ms, info, _ = oracle_sample(w, max_steps=args.steps)
+    step_s = info.pop("step_s")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": round(ms, 1), "unit": "ms", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(float(np.mean(step_s)) * 1e3, 2),
+        "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: {shape.L} layers, {shape.Hq}q/{shape.Hkv}kv heads, D {shape.D}, "
+                               f"block {shape.B}, history {list(w.hist)} tokens, {shape.n_new} new tokens",
+                   "mode": "oracle"},
+        "cpu_baseline": {"value": round(ms, 1), "unit": "ms", **info},
+        "e2e": {"value": round(ms, 1), "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    w.sess.close()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

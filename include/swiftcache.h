@@ -225,6 +225,16 @@ sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_al
                             const int32_t *hist_lens, const int32_t *cu_new, int32_t mode,
                             void *copy_stream, void *compute_stream);
 
+/* Per-kernel timing for measurement (bench.py's roofline): while enabled, every kernel
+ * launch is bracketed by CUDA events on the stream it is launched on.  Enabling clears
+ * earlier records.  sc_profile_collect waits for the recorded events and returns, per
+ * kernel kind (sc_kernel_kind_t), the summed device time in ms and the launch count.
+ * ms_sum, count: HOST arrays of SC_KERNEL_KINDS entries.                              */
+typedef enum { SC_KERNEL_GATHER = 0, SC_KERNEL_SCATTER = 1, SC_KERNEL_ATTENTION = 2,
+               SC_KERNEL_COMBINE = 3, SC_KERNEL_KINDS = 4 } sc_kernel_kind_t;
+sc_status_t sc_profile_enable(sc_pool_t *pool, int32_t on);
+sc_status_t sc_profile_collect(sc_pool_t *pool, double *ms_sum, int64_t *count);
+
 /* Number of kernels the library has launched since the pool was created (all kinds). */
 sc_status_t sc_launch_count(const sc_pool_t *pool, int64_t *n_launches);
 

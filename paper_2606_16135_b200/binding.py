@@ -37,7 +37,8 @@ SYMBOLS = [
     "sc_pool_info", "sc_cell_offset", "sc_lsc_offset", "sc_set_engine", "sc_set_split_tiles",
     "sc_alloc_blocks", "sc_free_blocks", "sc_num_free_blocks", "sc_append_blocks", "sc_store_prefix",
     "sc_read_tokens", "sc_load_layer", "sc_prefill_layer", "sc_load_layer_batched",
-    "sc_prefill_layer_batched", "sc_prefill_turn", "sc_launch_count",
+    "sc_prefill_layer_batched", "sc_prefill_turn", "sc_launch_count", "sc_profile_enable",
+    "sc_profile_collect",
 ]
 
 
@@ -97,6 +98,8 @@ def lib() -> C.CDLL:
         "sc_prefill_layer_batched": [vp, i32, vp, vp, vp, vp, i32, i32, i32p, i32p, i32, i32, vp, vp],
         "sc_prefill_turn": [vp, vp, vp, vp, vp, i32, vp, i32, i32, i32p, i32p, i32, vp, vp],
         "sc_launch_count": [vp, C.POINTER(i64)],
+        "sc_profile_enable": [vp, i32],
+        "sc_profile_collect": [vp, C.POINTER(C.c_double), C.POINTER(i64)],
     }
     for name, argtypes in sig.items():
         fn = getattr(L, name)
@@ -183,6 +186,17 @@ class Pool:
         n = C.c_int64()
         check(lib().sc_launch_count(self._h, C.byref(n)))
         return int(n.value)
+
+    def profile_enable(self, on: bool):
+        check(lib().sc_profile_enable(self._h, int(on)))
+
+    def profile_collect(self):
+        """{kind: (summed ms, launches)} for gather / scatter / attention / combine."""
+        ms = (C.c_double * 4)()
+        cnt = (C.c_int64 * 4)()
+        check(lib().sc_profile_collect(self._h, ms, cnt))
+        names = ("gather", "scatter", "attention", "combine")
+        return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(names)}
 
     # ---- allocator / tables (host)
     def alloc_blocks(self, n: int) -> np.ndarray:

@@ -43,6 +43,7 @@ struct ScBatch {
     int32_t lsc_off[SC_MAX_SEQS];     // first LSC block of each sequence
     int32_t cu_mt[SC_MAX_SEQS + 1];   // prefix sums of query M-tiles (engine specific)
     int32_t cu_blk[SC_MAX_SEQS + 1];  // prefix sums of blocks to copy (gather)
+    int32_t lsc_total;                // LSC blocks the whole batch occupies
 };
 
 __device__ __forceinline__ int64_t sc_phys_block(const ScKvView &v, const ScBatch &b, int s, int lb)
@@ -89,6 +90,27 @@ struct sc_pool {
     cudaEvent_t ev_fork = nullptr;
 
     int64_t launches = 0;
+
+    // per-kernel timing (sc_profile_enable / sc_profile_collect)
+    struct ProfRec { cudaEvent_t a, b; int kind; };
+    bool profiling = false;
+    std::vector<ProfRec> prof;
+};
+
+// Brackets one kernel launch with events on its own stream while profiling is on.
+struct ScProfScope {
+    sc_pool *p; cudaStream_t st; cudaEvent_t b = nullptr;
+    ScProfScope(sc_pool *pool, int kind, cudaStream_t s) : p(pool), st(s)
+    {
+        if (!p->profiling) return;
+        sc_pool::ProfRec r;
+        r.kind = kind;
+        if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
+        cudaEventRecord(r.a, st);
+        b = r.b;
+        p->prof.push_back(r);
+    }
+    ~ScProfScope() { if (b) cudaEventRecord(b, st); }
 };
 
 // error reporting (sc_api.cu): formats into the thread-local buffer of sc_last_error()

@@ -2,6 +2,8 @@
 // then kernel launches on the caller's stream.  No step of the path runs on the CPU.
 #include <string.h>
 
+#include <algorithm>
+
 #include "sc_internal.h"
 
 namespace {
@@ -72,13 +74,13 @@ sc_status_t make_batch(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, 
     b->cu_new[n_seq] = cu_new[n_seq];
     b->cu_mt[n_seq] = mt;
     b->cu_blk[n_seq] = blk;
-    for (int s = n_seq; s < SC_MAX_SEQS; ++s) b->lsc_off[s] = lsc;   // total, read by callers
+    b->lsc_total = lsc;
     if (cu_new[n_seq] > p->cfg.max_new_tokens)
         return sc_fail(SC_ERR_CAPACITY, "%d new tokens > max_new_tokens %d", cu_new[n_seq], p->cfg.max_new_tokens);
     return SC_OK;
 }
 
-int lsc_blocks_needed(const ScBatch &b) { return b.lsc_off[SC_MAX_SEQS - 1]; }
+int lsc_blocks_needed(const ScBatch &b) { return b.lsc_total; }
 
 }  // namespace
 
@@ -101,8 +103,11 @@ sc_status_t sc_store_prefix(sc_pool_t *pool, int32_t layer, const void *k, const
     b.n_seq = 1;
     b.hist[0] = start_token;
     b.cu_new[1] = n_tokens;
-    SC_CUDA(sc_launch_scatter(pool->g, k, v, b, pool_view(pool, layer, table_dev, n_table), nullptr,
-                              (cudaStream_t)stream));
+    {
+        ScProfScope ps(pool, SC_KERNEL_SCATTER, (cudaStream_t)stream);
+        SC_CUDA(sc_launch_scatter(pool->g, k, v, b, pool_view(pool, layer, table_dev, n_table), nullptr,
+                                  (cudaStream_t)stream));
+    }
     pool->launches += 1;
     return SC_OK;
 }
@@ -156,8 +161,11 @@ sc_status_t sc_load_layer_batched(sc_pool_t *pool, int32_t layer, const int32_t 
                        pool->cfg.lsc_blocks);
     int engine = pool->copy_engine;
     if (engine == SC_COPY_AUTO) engine = SC_COPY_LDG;
-    SC_CUDA(sc_launch_gather(pool->g, b, pool_view(pool, layer, tables_dev, max_blocks), lsc_view(pool, buf),
-                             engine, pool->n_sms, (cudaStream_t)stream));
+    {
+        ScProfScope ps(pool, SC_KERNEL_GATHER, (cudaStream_t)stream);
+        SC_CUDA(sc_launch_gather(pool->g, b, pool_view(pool, layer, tables_dev, max_blocks), lsc_view(pool, buf),
+                                 engine, pool->n_sms, (cudaStream_t)stream));
+    }
     pool->launches += (b.cu_blk[n_seq] > 0);
     return SC_OK;
 }
@@ -201,7 +209,10 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     const ScKvView lv = staged ? lsc_view(pool, buf) : pv;
 
     // 1. scatter (a5): pool, and the LSC tail in staged mode
-    SC_CUDA(sc_launch_scatter(pool->g, k_new, v_new, b, pv, staged ? &lv : nullptr, s));
+    {
+        ScProfScope ps(pool, SC_KERNEL_SCATTER, s);
+        SC_CUDA(sc_launch_scatter(pool->g, k_new, v_new, b, pv, staged ? &lv : nullptr, s));
+    }
     pool->launches += 1;
 
     // 2. attention (a6), split over the keys when that is needed to fill the machine
@@ -229,11 +240,17 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     a.split_tiles = split_tiles;
     a.n_splits = n_splits;
     a.total_new = total_new;
-    SC_CUDA(sc_launch_attn_mma(pool->g, b, a, s));
+    {
+        ScProfScope ps(pool, SC_KERNEL_ATTENTION, s);
+        SC_CUDA(sc_launch_attn_mma(pool->g, b, a, s));
+    }
     pool->launches += 1;
     // 3. combine (a7)
     if (n_splits > 1) {
-        SC_CUDA(sc_launch_combine(pool->g, b, a, tile_m, tile_n, s));
+        {
+            ScProfScope ps(pool, SC_KERNEL_COMBINE, s);
+            SC_CUDA(sc_launch_combine(pool->g, b, a, tile_m, tile_n, s));
+        }
         pool->launches += 1;
     }
     return SC_OK;
@@ -336,6 +353,30 @@ sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_al
     if (host_io) {   // join: the compute stream finishes last
         SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_d2h[(L - 1) & 1], 0));
         if (L >= 2) SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_d2h[(L - 2) & 1], 0));
+    }
+    return SC_OK;
+}
+
+sc_status_t sc_profile_enable(sc_pool_t *pool, int32_t on)
+{
+    if (!pool) return sc_fail(SC_ERR_INVALID_ARG, "pool is NULL");
+    if (pool->host_only) return sc_fail(SC_ERR_CUDA, "host-only pool");
+    for (auto &r : pool->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    pool->prof.clear();
+    pool->profiling = (on != 0);
+    return SC_OK;
+}
+
+sc_status_t sc_profile_collect(sc_pool_t *pool, double *ms_sum, int64_t *count)
+{
+    if (!pool || !ms_sum || !count) return sc_fail(SC_ERR_INVALID_ARG, "NULL argument");
+    for (int k = 0; k < SC_KERNEL_KINDS; ++k) { ms_sum[k] = 0; count[k] = 0; }
+    for (auto &r : pool->prof) {
+        SC_CUDA(cudaEventSynchronize(r.b));
+        float ms = 0;
+        SC_CUDA(cudaEventElapsedTime(&ms, r.a, r.b));
+        ms_sum[r.kind] += ms;
+        count[r.kind] += 1;
     }
     return SC_OK;
 }
