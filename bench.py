@@ -363,7 +363,7 @@ def run_ours(args):
     for name, rec in prof.items():
         if name in kernels:
             kernels[name]["share"] = round(rec[0] / tot, 4)
-    dom = max(prof, key=lambda n: prof[n][0])
+    dom = max((n for n in prof if work[n][1]), key=lambda n: prof[n][0])
     d_avg = avg(prof[dom])
     bound, amount = work[dom]
     traffic = None
