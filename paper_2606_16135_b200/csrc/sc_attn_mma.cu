@@ -282,6 +282,7 @@ sc_combine_kernel(ScGeom g, ScBatch b, ScAttnArgs a, int tile_m, int tile_n)
         const int64_t prow = ((int64_t)sp * a.total_new + grow) * g.Hq + h;
         const float m = a.part_ml[prow * 2], l = a.part_ml[prow * 2 + 1];
         const float wgt = (m == -INFINITY) ? 0.f : exp2f(m - M);
+        if (wgt == 0.f) continue;                  // O_s of such a split may never have been written
         W += wgt * l;
         const float *o = a.part_o + prow * D + lane * V;
 #pragma unroll

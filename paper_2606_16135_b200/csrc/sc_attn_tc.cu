@@ -1,0 +1,494 @@
+// sc_attn_tc.cu -- paged prefill attention, tcgen05 / TMEM engine (
+// each new token attends to all history tokens and to the new tokens up to
+// and including itself).
+//
+// One CTA owns a PAIR of 128-row query tiles of one query head (256 new tokens) and a
+// contiguous range of 128-token KV tiles (one split).  Warp roles:
+//   warp 0      producer : per KV tile, 8 + 8 bulk copies (cp.async.bulk, 4 KiB each) bring
+//                          the K and V chunks of the tile's 8 pool blocks -- found through the
+//                          block table -- into a 5-slot shared-memory ring.  The pool stores
+//                          chunks in the tensor core's 128B-swizzled operand order
+//                          (include/swiftcache.h), so a chunk is an MMA operand as it lands.
+//   warp 1      MMA      : one thread issues tcgen05.mma.  S_m = Q_m K^T (both operands in
+//                          shared memory, K-major) into TMEM; O_m += P_m V with P_m read from
+//                          TMEM and V as an MN-major shared-memory operand.
+//   warp 2      TMEM allocation (all 512 columns: S0 S1 O0 O1, 128 fp32 columns each)
+//   warps 4-7   softmax warpgroup of query tile 0: thread r owns row r.  tcgen05.ld S,
+//   warps 8-11  same for query tile 1            : mask, online softmax in registers with
+//                          lazy rescaling of O (only when the row max grows by > 2^8), P
+//                          rounded to bf16 and stored over S in TMEM, epilogue.
+// The two query tiles ping-pong on the tensor pipe: while warpgroup 0 does the softmax of
+// tile j, the pipe runs PV and QK^T of query tile 1.
+//
+// Work partitioning depends on logical positions only, so results are bit-identical under
+// any permutation of physical block ids, and staged attention is this same kernel run with
+// the identity table over the LSC.
+#include <cuda_bf16.h>
+
+#include "sc_internal.h"
+
+namespace {
+
+constexpr int kTM = 128;          // rows of one query tile
+constexpr int kPairM = 2 * kTM;   // rows a CTA owns
+constexpr int kTN = 128;          // KV tokens per tile (8 pool blocks)
+constexpr int kStages = 5;        // ring slots (each holds the K or the V half of a tile)
+constexpr int kThreads = 384;
+constexpr float kRescaleThreshold = 8.f;   // log2 units
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+
+// ------------------------------------------------------------------ mbarrier
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
+// A wait that cannot hang the GPU: after ~2 s of failed probes the kernel traps (surfaces as
+// SC_ERR_CUDA on the next call) instead of spinning forever on a protocol error.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    long long t0 = 0;
+    for (;;) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return;
+        const long long t = clock64();
+        if (t0 == 0) t0 = t;
+        else if (t - t0 > 4000000000ll) __trap();
+    }
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t smem_dst, const void *gsrc, uint32_t bytes, uint32_t bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        :: "r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar) : "memory");
+}
+
+// ------------------------------------------------------------------ tcgen05
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+// shared-memory matrix descriptor, 128-byte swizzle, version 1 (Blackwell)
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) |
+           ((uint64_t)(sbo_bytes >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+// instruction descriptor: bf16 x bf16 -> fp32, M = 128, A K-major
+__host__ __device__ constexpr uint32_t make_idesc(int n, int b_mn_major)
+{
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(n >> 3) << 17) |
+           ((uint32_t)(kTM >> 4) << 24);
+}
+__device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+        :: "r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+// arrives on `bar` when every tcgen05.mma issued so far by this thread has completed
+__device__ __forceinline__ void umma_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
+}
+
+// 32 lanes x 32 columns of 32-bit: thread i of the warp gets lane (base + i), columns col..col+31
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%32], "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
+        :: "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+           "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
+           "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
+           "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]),
+           "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
+{
+    __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t *>(&v);
+}
+__device__ __forceinline__ int seq_of(const int32_t *cu, int n_seq, int x)
+{
+    int s = 0;
+    while (s + 1 < n_seq && x >= cu[s + 1]) ++s;
+    return s;
+}
+
+// shared-memory plan (offsets from the 1024-byte aligned base)
+template <int D>
+struct Plan {
+    static constexpr int NH = D / 64;
+    static constexpr int kChunk = 16 * D * 2;          // one (block, head) chunk
+    static constexpr int kQTile = kTM * D * 2;         // one query tile, swizzled like a K tile
+    static constexpr int kSlot = kTN * D * 2;          // K (or V) of one KV tile = 8 chunks
+    static constexpr int kQOff = 0;
+    static constexpr int kRingOff = 2 * kQTile;
+    static constexpr int kBarOff = kRingOff + kStages * kSlot;
+    static constexpr int kBytes = kBarOff + 256 + 1024;   // + barriers + alignment slack
+};
+
+struct Bars {                       // at Plan::kBarOff
+    uint64_t full[kStages], empty[kStages];
+    uint64_t s_ready[2];            // MMA -> softmax warpgroup m: S_m written (and earlier PV_m done)
+    uint64_t p_ready[2];            // softmax warpgroup m -> MMA: P_m stored, O_m rescaled
+    uint64_t q_ready[2];            // Q_m in shared memory
+    uint32_t tmem_base;
+};
+
+template <int D>
+__global__ void __launch_bounds__(kThreads, 1)
+sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
+{
+    using P = Plan<D>;
+    constexpr int NH = P::NH;
+    extern __shared__ char smem_raw[];
+    const uint32_t raw_u32 = smem_u32(smem_raw);
+    const uint32_t base = (raw_u32 + 1023u) & ~1023u;
+    char *smem = smem_raw + (base - raw_u32);
+    Bars *bars = reinterpret_cast<Bars *>(smem + P::kBarOff);
+
+    // ---- which work is this CTA's (all of it warp- and CTA-uniform) ----
+    const int split = blockIdx.x, h = blockIdx.y, gp = blockIdx.z;
+    const int s = seq_of(b.cu_mt, b.n_seq, gp);
+    const int pair = gp - b.cu_mt[s];
+    const int n_s = b.cu_new[s + 1] - b.cu_new[s];
+    const int T_h = b.hist[s];
+    const int tok0 = pair * kPairM;
+    int rows[2], need[2], nt[2];
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+        rows[m] = max(0, min(kTM, n_s - tok0 - m * kTM));
+        need[m] = rows[m] > 0 ? (T_h + tok0 + m * kTM + rows[m] + kTN - 1) / kTN : 0;
+    }
+    const int need_max = max(need[0], need[1]);
+    const int t_begin = split * a.split_tiles;
+    if (t_begin >= need_max) return;
+    const int t_end = min(t_begin + a.split_tiles, need_max);
+    const int nt_max = t_end - t_begin;
+#pragma unroll
+    for (int m = 0; m < 2; ++m) nt[m] = max(0, min(t_end, need[m]) - t_begin);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t bar_full = smem_u32(&bars->full[0]), bar_empty = smem_u32(&bars->empty[0]);
+    const uint32_t bar_s = smem_u32(&bars->s_ready[0]), bar_p = smem_u32(&bars->p_ready[0]);
+    const uint32_t bar_q = smem_u32(&bars->q_ready[0]);
+    const uint32_t q_smem = base + P::kQOff, ring = base + P::kRingOff;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < kStages; ++i) { mbar_init(bar_full + 8 * i, 1); mbar_init(bar_empty + 8 * i, 1); }
+        for (int m = 0; m < 2; ++m) {
+            mbar_init(bar_s + 8 * m, 1);
+            mbar_init(bar_p + 8 * m, kTM);
+            mbar_init(bar_q + 8 * m, kTM);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;"
+                     :: "r"(smem_u32(&bars->tmem_base)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = bars->tmem_base;
+
+    if (warp == 0) {
+        // =============================== producer ===============================
+        if (lane == 0) {
+            const int nblk = (T_h + n_s + 15) >> 4;
+            const int hk = h / (g.Hq / g.Hkv);
+            const int64_t off_kv[2] = {(int64_t)hk * P::kChunk, (int64_t)(g.Hkv + hk) * P::kChunk};
+            for (int jj = 0; jj < nt_max; ++jj) {
+                const int j = t_begin + jj;
+                const char *blk[8];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    const int lb = min(j * 8 + c, nblk - 1);
+                    blk[c] = a.kv.base + sc_phys_block(a.kv, b, s, lb) * a.kv.block_stride;
+                }
+#pragma unroll
+                for (int kv = 0; kv < 2; ++kv) {
+                    const int it = 2 * jj + kv, slot = it % kStages;
+                    mbar_wait(bar_empty + 8 * slot, ((it / kStages) & 1) ^ 1);
+                    mbar_expect_tx(bar_full + 8 * slot, P::kSlot);
+#pragma unroll
+                    for (int c = 0; c < 8; ++c)
+                        bulk_g2s(ring + slot * P::kSlot + c * P::kChunk, blk[c] + off_kv[kv], P::kChunk,
+                                 bar_full + 8 * slot);
+                }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 1) {
+        // =============================== MMA issuer ===============================
+        if (lane == 0) {
+            constexpr uint32_t idesc_qk = make_idesc(kTN, 0), idesc_pv = make_idesc(D, 1);
+            auto issue_qk = [&](int m, uint32_t kslot) {
+#pragma unroll
+                for (int hf = 0; hf < NH; ++hf)
+#pragma unroll
+                    for (int kk = 0; kk < 4; ++kk) {
+                        const uint32_t o = hf * 1024 + kk * 32;
+                        umma_ss(tmem + m * 128, make_desc(q_smem + m * P::kQTile + o, 16, NH * 1024),
+                                make_desc(kslot + o, 16, NH * 1024), idesc_qk, (hf | kk) != 0);
+                    }
+            };
+            auto issue_pv = [&](int m, uint32_t vslot, bool acc) {
+#pragma unroll
+                for (int kk = 0; kk < 8; ++kk)
+                    umma_ts(tmem + 256 + m * 128, tmem + m * 128 + kk * 8,
+                            make_desc(vslot + kk * P::kChunk, 1024, NH * 1024), idesc_pv, acc || kk != 0);
+            };
+            auto slot_addr = [&](int it) { return ring + (it % kStages) * P::kSlot; };
+            auto wait_full = [&](int it) {
+                mbar_wait(bar_full + 8 * (it % kStages), (it / kStages) & 1);
+                tc_fence_after();
+            };
+            // prologue: S_m = Q_m K_0^T
+            wait_full(0);
+#pragma unroll
+            for (int m = 0; m < 2; ++m)
+                if (nt[m] > 0) {
+                    mbar_wait(bar_q + 8 * m, 0);
+                    issue_qk(m, slot_addr(0));
+                    umma_commit(bar_s + 8 * m);
+                }
+            umma_commit(bar_empty + 8 * (0 % kStages));
+            for (int jj = 0; jj < nt_max; ++jj) {
+                const int itv = 2 * jj + 1, itk = 2 * jj + 2;
+                wait_full(itv);
+                bool k_waited = false;
+#pragma unroll
+                for (int m = 0; m < 2; ++m) {
+                    if (jj >= nt[m]) continue;
+                    mbar_wait(bar_p + 8 * m, jj & 1);
+                    tc_fence_after();
+                    issue_pv(m, slot_addr(itv), jj > 0);
+                    if (jj + 1 < nt[m]) {
+                        if (!k_waited) { wait_full(itk); k_waited = true; }
+                        issue_qk(m, slot_addr(itk));
+                    }
+                    umma_commit(bar_s + 8 * m);      // S_m(jj+1) ready, or: O_m final
+                }
+                umma_commit(bar_empty + 8 * (itv % kStages));
+                if (jj + 1 < nt_max) umma_commit(bar_empty + 8 * (itk % kStages));
+            }
+        }
+        __syncwarp();
+    } else if (warp >= 4) {
+        // =============================== softmax warpgroups ===============================
+        const int m = (warp - 4) >> 2, wl = warp & 3;
+        const int r = wl * 32 + lane;                         // row of the query tile = TMEM lane
+        const int t128 = threadIdx.x - 128 - m * kTM;         // 0..127 inside the warpgroup
+        const int row0 = tok0 + m * kTM;                      // first new-token index of the tile
+        const int64_t grow = (int64_t)b.cu_new[s] + row0 + r; // packed row of (s, token)
+        if (nt[m] > 0) {
+            // ---- Q_m -> shared memory, swizzled exactly like a K tile ----
+            constexpr int CPR = D / 8;                        // 16-byte units per row
+            const char *qg = (const char *)a.q;
+            const uint32_t qs = q_smem + m * P::kQTile;
+#pragma unroll 4
+            for (int it = 0; it < CPR; ++it) {
+                const int u = it * kTM + t128;
+                const int row = u / CPR, c16 = u % CPR, hf = c16 >> 3, c = c16 & 7;
+                int4 v = make_int4(0, 0, 0, 0);
+                if (row < rows[m])
+                    v = __ldg(reinterpret_cast<const int4 *>(
+                        qg + (((int64_t)b.cu_new[s] + row0 + row) * g.Hq + h) * (D * 2) + c16 * 16));
+                const uint32_t dst = qs + (row >> 3) * (NH * 1024) + hf * 1024 + (row & 7) * 128 + ((c ^ (row & 7)) << 4);
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" :: "r"(dst), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_arrive(bar_q + 8 * m);
+        }
+
+        const float sl = 1.4426950408889634f * rsqrtf((float)D);      // log2(e)/sqrt(D)
+        const uint32_t lane_base = (uint32_t)(wl * 32) << 16;
+        const uint32_t s_addr = tmem + lane_base + m * 128, o_addr = tmem + lane_base + 256 + m * 128;
+        float m_used = -INFINITY, l_run = 0.f;
+        for (int jj = 0; jj < nt[m]; ++jj) {
+            const int j = t_begin + jj;
+            mbar_wait(bar_s + 8 * m, jj & 1);
+            tc_fence_after();
+            uint32_t sv[kTN];
+#pragma unroll
+            for (int c4 = 0; c4 < kTN / 32; ++c4)
+                tmem_ld32(s_addr + c4 * 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[c4 * 32]));
+            tmem_ld_wait();
+            if (j * kTN + kTN - 1 > T_h + row0) {               // tile reaches past the first row's limit
+                const int limit = T_h + row0 + r - j * kTN;     // last visible column of this row
+#pragma unroll
+                for (int c = 0; c < kTN; ++c)
+                    if (c > limit) sv[c] = 0xff800000u;         // -inf
+            }
+            float mx = -INFINITY;
+#pragma unroll
+            for (int c = 0; c < kTN; ++c) mx = fmaxf(mx, __uint_as_float(sv[c]));
+            const float m_new = fmaxf(m_used, mx);
+            const bool grow_max = (m_new - m_used) * sl > kRescaleThreshold;   // false for -inf - -inf (NaN)
+            if (jj == 0) {
+                m_used = m_new;                                 // O_m not accumulated yet
+            } else if (__any_sync(0xffffffffu, grow_max)) {
+                const float alpha = grow_max ? exp2f((m_used - m_new) * sl) : 1.f;
+                if (grow_max) m_used = m_new;
+                l_run *= alpha;
+#pragma unroll
+                for (int c4 = 0; c4 < D / 32; ++c4) {
+                    uint32_t o[32];
+                    tmem_ld32(o_addr + c4 * 32, o);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
+                    tmem_st32(o_addr + c4 * 32, o);
+                }
+            }
+            const float msl = (m_used == -INFINITY) ? 0.f : m_used * sl;
+            float rs = 0.f;
+#pragma unroll
+            for (int c = 0; c < kTN / 2; ++c) {
+                const float p0 = exp2f(fmaf(__uint_as_float(sv[2 * c]), sl, -msl));
+                const float p1 = exp2f(fmaf(__uint_as_float(sv[2 * c + 1]), sl, -msl));
+                rs += p0 + p1;
+                sv[c] = pack_bf16(p0, p1);                      // in place: c <= 2c
+            }
+            l_run += rs;
+            tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&sv[0]));
+            tmem_st32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[32]));
+            tmem_st_wait();
+            tc_fence_before();
+            mbar_arrive(bar_p + 8 * m);
+        }
+
+        // ---- epilogue ----
+        if (nt[m] > 0) {
+            mbar_wait(bar_s + 8 * m, nt[m] & 1);
+            tc_fence_after();
+            const bool valid = r < rows[m];
+            if (a.n_splits == 1) {
+                const float inv = __fdividef(1.f, l_run);
+                char *orow = (char *)a.out + (grow * g.Hq + h) * (D * 2);
+#pragma unroll
+                for (int c4 = 0; c4 < D / 32; ++c4) {
+                    uint32_t o[32];
+                    tmem_ld32(o_addr + c4 * 32, o);
+                    tmem_ld_wait();
+                    if (valid) {
+#pragma unroll
+                        for (int q4 = 0; q4 < 4; ++q4) {
+                            int4 v;
+                            v.x = pack_bf16(__uint_as_float(o[q4 * 8 + 0]) * inv, __uint_as_float(o[q4 * 8 + 1]) * inv);
+                            v.y = pack_bf16(__uint_as_float(o[q4 * 8 + 2]) * inv, __uint_as_float(o[q4 * 8 + 3]) * inv);
+                            v.z = pack_bf16(__uint_as_float(o[q4 * 8 + 4]) * inv, __uint_as_float(o[q4 * 8 + 5]) * inv);
+                            v.w = pack_bf16(__uint_as_float(o[q4 * 8 + 6]) * inv, __uint_as_float(o[q4 * 8 + 7]) * inv);
+                            *reinterpret_cast<int4 *>(orow + c4 * 64 + q4 * 16) = v;
+                        }
+                    }
+                }
+            } else {
+                const int64_t prow = ((int64_t)split * a.total_new + grow) * g.Hq + h;
+                float *orow = a.part_o + prow * D;
+#pragma unroll
+                for (int c4 = 0; c4 < D / 32; ++c4) {
+                    uint32_t o[32];
+                    tmem_ld32(o_addr + c4 * 32, o);
+                    tmem_ld_wait();
+                    if (valid) {
+#pragma unroll
+                        for (int q4 = 0; q4 < 8; ++q4)
+                            *reinterpret_cast<uint4 *>(orow + c4 * 32 + q4 * 4) =
+                                make_uint4(o[q4 * 4], o[q4 * 4 + 1], o[q4 * 4 + 2], o[q4 * 4 + 3]);
+                    }
+                }
+                if (valid) {
+                    a.part_ml[prow * 2 + 0] = m_used * sl;      // log2 units; may be -inf
+                    a.part_ml[prow * 2 + 1] = l_run;
+                }
+            }
+        } else if (a.n_splits > 1 && r < rows[m]) {
+            // the tile exists but sees none of this split's keys: weight 0 in the combine
+            const int64_t prow = ((int64_t)split * a.total_new + grow) * g.Hq + h;
+            a.part_ml[prow * 2 + 0] = -INFINITY;
+            a.part_ml[prow * 2 + 1] = 0.f;
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" :: "r"(tmem) : "memory");
+}
+
+}  // namespace
+
+int sc_tc_tile_m() { return kPairM; }
+int sc_tc_tile_n() { return kTN; }
+
+cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st)
+{
+    const int total_pairs = b.cu_mt[b.n_seq];
+    if (total_pairs == 0) return cudaSuccess;
+    dim3 grid((unsigned)a.n_splits, (unsigned)g.Hq, (unsigned)total_pairs);
+    cudaError_t e;
+    if (g.D == 128) {
+        static bool set = false;
+        if (!set) {
+            e = cudaFuncSetAttribute(sc_attn_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<128>::kBytes);
+            if (e != cudaSuccess) return e;
+            set = true;
+        }
+        sc_attn_tc_kernel<128><<<grid, kThreads, Plan<128>::kBytes, st>>>(g, b, a);
+    } else {
+        static bool set = false;
+        if (!set) {
+            e = cudaFuncSetAttribute(sc_attn_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<64>::kBytes);
+            if (e != cudaSuccess) return e;
+            set = true;
+        }
+        sc_attn_tc_kernel<64><<<grid, kThreads, Plan<64>::kBytes, st>>>(g, b, a);
+    }
+    return cudaGetLastError();
+}

@@ -140,5 +140,9 @@ struct ScAttnArgs {
 int sc_mma_tile_m();   // query rows per CTA of the mma.sync engine
 int sc_mma_tile_n();   // KV tokens per tile
 cudaError_t sc_launch_attn_mma(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st);
+// sc_attn_tc.cu  (tcgen05 / TMEM engine): a CTA owns a pair of 128-row query tiles
+int sc_tc_tile_m();
+int sc_tc_tile_n();
+cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st);
 cudaError_t sc_launch_combine(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, int tile_m,
                               int tile_n, cudaStream_t st);

@@ -82,6 +82,38 @@ sc_status_t make_batch(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, 
 
 int lsc_blocks_needed(const ScBatch &b) { return b.lsc_total; }
 
+// KV tiles per split.  Every (query tile group, head) needs ceil(tiles/split) CTAs of up to
+// `split` tiles each; the grid runs in waves of n_sms*ctas_per_sm CTAs, and a CTA costs its
+// tiles plus a fixed overhead (prologue, epilogue, partial write + combine read).  Pick the
+// split with the smallest  waves * (split + overhead).  Depends on logical lengths only.
+int choose_split_tiles(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, const int32_t *cu_new,
+                       int tile_m, int tile_n, int ctas_per_sm)
+{
+    int max_tiles = 1;
+    for (int i = 0; i < n_seq; ++i)
+        max_tiles = std::max(max_tiles, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), tile_n));
+    const int64_t wave = (int64_t)p->n_sms * ctas_per_sm;
+    const double overhead = 2.5;
+    int best = max_tiles;
+    double best_cost = 1e30;
+    for (int n_sp = 1; n_sp <= p->max_splits; ++n_sp) {
+        const int split = ceil_div(max_tiles, n_sp);
+        if (n_sp > 1 && ceil_div(max_tiles, split) != n_sp) continue;     // same split as a smaller n_sp
+        int64_t ctas = 0;
+        for (int i = 0; i < n_seq; ++i) {
+            const int n = cu_new[i + 1] - cu_new[i];
+            for (int mt = 0; mt * tile_m < n; ++mt) {
+                const int kmax = hist_lens[i] + std::min(n, (mt + 1) * tile_m);
+                ctas += (int64_t)p->g.Hq * ceil_div(ceil_div(kmax, tile_n), split);
+            }
+        }
+        const double waves = (double)((ctas + wave - 1) / wave);
+        const double cost = waves * (split + overhead) + (n_sp > 1 ? 0.5 : 0.0);
+        if (cost < best_cost - 1e-9) { best_cost = cost; best = split; }
+    }
+    return std::max(best, 1);
+}
+
 }  // namespace
 
 extern "C" {
@@ -192,9 +224,9 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     if (mode != SC_ATTN_STAGED && mode != SC_ATTN_FUSED) return sc_fail(SC_ERR_INVALID_ARG, "mode %d", mode);
     if (buf < 0 || buf > 1) return sc_fail(SC_ERR_INVALID_ARG, "buf %d not in {0,1}", buf);
     int engine = pool->attn_engine;
-    if (engine == SC_ENGINE_AUTO) engine = SC_ENGINE_MMA_SYNC;
-    if (engine == SC_ENGINE_TCGEN05) return sc_fail(SC_ERR_UNSUPPORTED, "tcgen05 engine not built");
-    const int tile_m = sc_mma_tile_m(), tile_n = sc_mma_tile_n();
+    if (engine == SC_ENGINE_AUTO) engine = SC_ENGINE_TCGEN05;
+    const bool tc = (engine == SC_ENGINE_TCGEN05);
+    const int tile_m = tc ? sc_tc_tile_m() : sc_mma_tile_m(), tile_n = tc ? sc_tc_tile_n() : sc_mma_tile_n();
     ScBatch b;
     st = make_batch(pool, n_seq, hist_lens, cu_new, max_blocks, tile_m, &b);
     if (st) return st;
@@ -216,16 +248,11 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     pool->launches += 1;
 
     // 2. attention (a6), split over the keys when that is needed to fill the machine
+    int split_tiles = pool->split_tiles_override;
+    if (split_tiles <= 0) split_tiles = choose_split_tiles(pool, n_seq, hist_lens, cu_new, tile_m, tile_n, tc ? 1 : 3);
     int max_tiles = 1;
     for (int i = 0; i < n_seq; ++i)
         max_tiles = std::max(max_tiles, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), tile_n));
-    const int base_ctas = pool->g.Hq * b.cu_mt[n_seq];
-    int split_tiles = pool->split_tiles_override;
-    if (split_tiles <= 0) {
-        int want = ceil_div(3 * pool->n_sms, base_ctas);
-        want = std::max(1, std::min(want, pool->max_splits));
-        split_tiles = std::max(ceil_div(max_tiles, want), 4);
-    }
     int n_splits = ceil_div(max_tiles, split_tiles);
     if (n_splits > pool->max_splits) {
         split_tiles = ceil_div(max_tiles, pool->max_splits);
@@ -242,7 +269,7 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     a.total_new = total_new;
     {
         ScProfScope ps(pool, SC_KERNEL_ATTENTION, s);
-        SC_CUDA(sc_launch_attn_mma(pool->g, b, a, s));
+        SC_CUDA(tc ? sc_launch_attn_tc(pool->g, b, a, s) : sc_launch_attn_mma(pool->g, b, a, s));
     }
     pool->launches += 1;
     // 3. combine (a7)

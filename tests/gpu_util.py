@@ -30,13 +30,14 @@ class Case:
     """One conversation in one pool, mirrored in the oracle's pool."""
 
     def __init__(self, L, Hq, Hkv, D, T_h, n, NB, seed, variant="normal", identity=False, perm_id=1,
-                 lsc_extra=2, split_tiles=0, max_new=None):
+                 lsc_extra=2, split_tiles=0, max_new=None, engine=sc.SC_ENGINE_AUTO):
         self.L, self.Hq, self.Hkv, self.D, self.T_h, self.n = L, Hq, Hkv, D, T_h, n
         B = 16
         nb_total = O.blocks_for(T_h + n, B)
         assert NB >= nb_total
         self.table = I.block_table(perm_id, NB, nb_total, identity=identity)
         self.sess = Session(L, Hq, Hkv, D, B, NB, nb_total + lsc_extra, max_new or max(n, 1))
+        self.sess.pool.set_engine(engine, sc.SC_COPY_AUTO)
         if split_tiles:
             self.sess.pool.set_split_tiles(split_tiles)
         self.opool = O.Pool(L, Hkv, D, B, NB)
