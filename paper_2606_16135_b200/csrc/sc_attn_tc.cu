@@ -24,6 +24,7 @@
 // any permutation of physical block ids, and staged attention is this same kernel run with
 // the identity table over the LSC.
 #include <cuda_bf16.h>
+#include <stdlib.h>
 
 #include "sc_internal.h"
 
@@ -77,6 +78,13 @@ __device__ __forceinline__ void bulk_g2s(uint32_t smem_dst, const void *gsrc, ui
     asm volatile(
         "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
         :: "r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar) : "memory");
+}
+
+// all threads of all CTAs of the cluster; release / acquire at cluster scope (global writes included)
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
 // ------------------------------------------------------------------ tcgen05
@@ -178,6 +186,17 @@ struct Bars {                       // at Plan::kBarOff
     uint32_t tmem_base;
 };
 
+#ifdef SC_TC_PROBE
+__constant__ int sc_probe_flags;
+__device__ long long sc_tl[256][64];
+#define PROBE(bit) (sc_probe_flags & (1 << (bit)))
+#define TL(i) do { const int cta_ = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z); \
+                   if (cta_ < 256) sc_tl[cta_][(i)] = clock64(); } while (0)
+#else
+#define PROBE(bit) 0
+#define TL(i) do { } while (0)
+#endif
+
 template <int D>
 __global__ void __launch_bounds__(kThreads, 1)
 sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
@@ -205,13 +224,17 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     }
     const int need_max = max(need[0], need[1]);
     const int t_begin = split * a.split_tiles;
-    if (t_begin >= need_max) return;
+    if (t_begin >= need_max) {                   // no keys for this split: only keep the cluster barriers whole
+        if (a.cluster_combine) { cluster_sync_all(); cluster_sync_all(); }
+        return;
+    }
     const int t_end = min(t_begin + a.split_tiles, need_max);
     const int nt_max = t_end - t_begin;
 #pragma unroll
     for (int m = 0; m < 2; ++m) nt[m] = max(0, min(t_end, need[m]) - t_begin);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) TL(0);
     const uint32_t bar_full = smem_u32(&bars->full[0]), bar_empty = smem_u32(&bars->empty[0]);
     const uint32_t bar_s = smem_u32(&bars->s_ready[0]), bar_p = smem_u32(&bars->p_ready[0]);
     const uint32_t bar_q = smem_u32(&bars->q_ready[0]);
@@ -235,7 +258,12 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = bars->tmem_base;
+    if (threadIdx.x == 128) TL(1);
+    float fin_m = -INFINITY, fin_l = 0.f;      // softmax threads: final (m in log2 units, l) of their row
 
+    // registers: the producer / MMA warpgroup gives most of its share to the softmax warpgroups
+    if (warp < 4) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
     if (warp == 0) {
         // =============================== producer ===============================
         if (lane == 0) {
@@ -254,6 +282,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 for (int kv = 0; kv < 2; ++kv) {
                     const int it = 2 * jj + kv, slot = it % kStages;
                     mbar_wait(bar_empty + 8 * slot, ((it / kStages) & 1) ^ 1);
+                    if (PROBE(4)) { mbar_arrive(bar_full + 8 * slot); continue; }
                     mbar_expect_tx(bar_full + 8 * slot, P::kSlot);
 #pragma unroll
                     for (int c = 0; c < 8; ++c)
@@ -268,6 +297,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         if (lane == 0) {
             constexpr uint32_t idesc_qk = make_idesc(kTN, 0), idesc_pv = make_idesc(D, 1);
             auto issue_qk = [&](int m, uint32_t kslot) {
+                if (PROBE(3)) return;
 #pragma unroll
                 for (int hf = 0; hf < NH; ++hf)
 #pragma unroll
@@ -278,6 +308,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     }
             };
             auto issue_pv = [&](int m, uint32_t vslot, bool acc) {
+                if (PROBE(2)) return;
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk)
                     umma_ts(tmem + 256 + m * 128, tmem + m * 128 + kk * 8,
@@ -319,8 +350,10 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             }
         }
         __syncwarp();
-    } else if (warp >= 4) {
+    }
+    } else {
         // =============================== softmax warpgroups ===============================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
         const int m = (warp - 4) >> 2, wl = warp & 3;
         const int r = wl * 32 + lane;                         // row of the query tile = TMEM lane
         const int t128 = threadIdx.x - 128 - m * kTM;         // 0..127 inside the warpgroup
@@ -331,7 +364,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             constexpr int CPR = D / 8;                        // 16-byte units per row
             const char *qg = (const char *)a.q;
             const uint32_t qs = q_smem + m * P::kQTile;
-#pragma unroll 4
+#pragma unroll
             for (int it = 0; it < CPR; ++it) {
                 const int u = it * kTM + t128;
                 const int row = u / CPR, c16 = u % CPR, hf = c16 >> 3, c = c16 & 7;
@@ -344,6 +377,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             mbar_arrive(bar_q + 8 * m);
+            if (threadIdx.x == 128) TL(2);
         }
 
         const float sl = 1.4426950408889634f * rsqrtf((float)D);      // log2(e)/sqrt(D)
@@ -354,6 +388,9 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             const int j = t_begin + jj;
             mbar_wait(bar_s + 8 * m, jj & 1);
             tc_fence_after();
+            if (threadIdx.x == 128 && jj < 12) TL(3 + 2 * jj);
+            if (threadIdx.x == 256 && jj < 12) TL(40 + jj);
+            if (PROBE(1)) { tc_fence_before(); mbar_arrive(bar_p + 8 * m); continue; }
             uint32_t sv[kTN];
 #pragma unroll
             for (int c4 = 0; c4 < kTN / 32; ++c4)
@@ -365,9 +402,21 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 for (int c = 0; c < kTN; ++c)
                     if (c > limit) sv[c] = 0xff800000u;         // -inf
             }
-            float mx = -INFINITY;
+            if (PROBE(0)) {
+                tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&sv[0]));
+                tmem_st32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[32]));
+                tmem_st_wait();
+                tc_fence_before();
+                mbar_arrive(bar_p + 8 * m);
+                continue;
+            }
+            float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};     // 4 chains: ILP
 #pragma unroll
-            for (int c = 0; c < kTN; ++c) mx = fmaxf(mx, __uint_as_float(sv[c]));
+            for (int c = 0; c < kTN; c += 8)
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    mx4[k] = fmaxf(mx4[k], fmaxf(__uint_as_float(sv[c + 2 * k]), __uint_as_float(sv[c + 2 * k + 1])));
+            const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
             const float m_new = fmaxf(m_used, mx);
             const bool grow_max = (m_new - m_used) * sl > kRescaleThreshold;   // false for -inf - -inf (NaN)
             if (jj == 0) {
@@ -387,28 +436,34 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 }
             }
             const float msl = (m_used == -INFINITY) ? 0.f : m_used * sl;
-            float rs = 0.f;
+            float rs4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
             for (int c = 0; c < kTN / 2; ++c) {
                 const float p0 = exp2f(fmaf(__uint_as_float(sv[2 * c]), sl, -msl));
                 const float p1 = exp2f(fmaf(__uint_as_float(sv[2 * c + 1]), sl, -msl));
-                rs += p0 + p1;
+                rs4[c & 3] += p0 + p1;
                 sv[c] = pack_bf16(p0, p1);                      // in place: c <= 2c
             }
-            l_run += rs;
+            l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
             tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&sv[0]));
             tmem_st32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[32]));
             tmem_st_wait();
             tc_fence_before();
             mbar_arrive(bar_p + 8 * m);
+            if (threadIdx.x == 128 && jj < 12) TL(4 + 2 * jj);
         }
 
+        fin_m = m_used * sl;
+        fin_l = l_run;
         // ---- epilogue ----
         if (nt[m] > 0) {
             mbar_wait(bar_s + 8 * m, nt[m] & 1);
             tc_fence_after();
+            if (threadIdx.x == 128) TL(30);
             const bool valid = r < rows[m];
-            if (a.n_splits == 1) {
+            if (a.cluster_combine) {
+                // O_m stays in TMEM until the cluster exchange below
+            } else if (a.n_splits == 1) {
                 const float inv = __fdividef(1.f, l_run);
                 char *orow = (char *)a.out + (grow * g.Hq + h) * (D * 2);
 #pragma unroll
@@ -448,7 +503,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     a.part_ml[prow * 2 + 1] = l_run;
                 }
             }
-        } else if (a.n_splits > 1 && r < rows[m]) {
+        } else if (a.n_splits > 1 && !a.cluster_combine && r < rows[m]) {
             // the tile exists but sees none of this split's keys: weight 0 in the combine
             const int64_t prow = ((int64_t)split * a.total_new + grow) * g.Hq + h;
             a.part_ml[prow * 2 + 0] = -INFINITY;
@@ -456,6 +511,93 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         }
     }
 
+    // ---- split-KV combine (a7), in kernel.  The CTAs of one (query tile pair, head) form a
+    //      thread-block cluster, one CTA per split.  Each CTA is responsible for a slice of the
+    //      pair's rows: every CTA sends the other CTAs' slices of its unnormalised partial
+    //      (m, l, O) straight from TMEM into their shared memory (DSMEM), and merges what it
+    //      receives in split order, so the result does not depend on timing. ----
+    if (a.cluster_combine) {
+        constexpr int CH = D / 4;                                  // 16-byte chunks per fp32 row
+        const int ns = (need_max + a.split_tiles - 1) / a.split_tiles;     // CTAs that hold keys
+        const int nrows = min(kPairM, n_s - tok0);
+        const int per = (nrows + ns - 1) / ns;                     // rows per CTA
+        const uint32_t recv_o = ring, recv_ml = ring + (kPairM + 8) * D * 4;   // [src][per][D] fp32, [src][per] (m, l)
+        cluster_sync_all();                  // every CTA of the cluster is done with its ring
+        if (threadIdx.x == 128) TL(31);
+        if (warp >= 4) {
+            const int m = (warp - 4) >> 2, wl = warp & 3;
+            const int prow = m * kTM + wl * 32 + lane;             // row of the pair
+            const bool valid = prow < nrows;
+            const int dst = valid ? prow / per : 0, i = prow - dst * per;
+            const uint32_t slot = (uint32_t)(split * per + i);
+            uint32_t rem_o, rem_ml;
+            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rem_o) : "r"(recv_o + slot * (D * 4)), "r"(dst));
+            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rem_ml) : "r"(recv_ml + slot * 8), "r"(dst));
+            if (valid)
+                asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" :: "r"(rem_ml), "f"(nt[m] > 0 ? fin_m : -INFINITY),
+                             "f"(nt[m] > 0 ? fin_l : 0.f) : "memory");
+            if (nt[m] > 0) {
+                const uint32_t o_addr = tmem + ((uint32_t)(wl * 32) << 16) + 256 + m * 128;
+                const uint32_t key = (uint32_t)prow & (CH - 1);
+#pragma unroll
+                for (int c4 = 0; c4 < D / 32; ++c4) {
+                    uint32_t o[32];
+                    tmem_ld32(o_addr + c4 * 32, o);
+                    tmem_ld_wait();
+                    if (valid) {
+#pragma unroll
+                        for (int q = 0; q < 8; ++q)
+                            asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};"
+                                         :: "r"(rem_o + ((((uint32_t)(c4 * 8 + q)) ^ key) << 4)), "r"(o[q * 4]), "r"(o[q * 4 + 1]),
+                                            "r"(o[q * 4 + 2]), "r"(o[q * 4 + 3]) : "memory");
+                    }
+                }
+            }
+        }
+        if (threadIdx.x == 128) TL(32);
+        cluster_sync_all();                  // all partials have landed
+        if (threadIdx.x == 128) TL(34);
+        if (warp >= 4) {
+            constexpr int RW = 32 / CH;                            // rows a warp handles at once
+            const int w8 = warp - 4, pch = lane % CH;
+            const int r_begin = split * per, n_mine = min(nrows, r_begin + per) - r_begin;
+            for (int i = w8 * RW + lane / CH; i < n_mine; i += 8 * RW) {
+                const int prow = r_begin + i;
+                float2 ml[8];
+                float M = -INFINITY;
+#pragma unroll
+                for (int sp = 0; sp < 8; ++sp) {
+                    ml[sp] = make_float2(-INFINITY, 0.f);
+                    if (sp < ns)
+                        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(ml[sp].x), "=f"(ml[sp].y)
+                                     : "r"(recv_ml + (uint32_t)(sp * per + i) * 8));
+                    M = fmaxf(M, ml[sp].x);
+                }
+                float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                float W = 0.f;
+#pragma unroll
+                for (int sp = 0; sp < 8; ++sp) {
+                    const float wgt = (ml[sp].x == -INFINITY) ? 0.f : exp2f(ml[sp].x - M);
+                    if (wgt != 0.f) {                   // an unweighted split sent no O
+                        float4 v;
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                                     : "r"(recv_o + (uint32_t)(sp * per + i) * (D * 4) + pch * 16));
+                        W += wgt * ml[sp].y;
+                        acc.x += wgt * v.x; acc.y += wgt * v.y; acc.z += wgt * v.z; acc.w += wgt * v.w;
+                    }
+                }
+                const float inv = __fdividef(1.f, W);
+                uint2 o2;
+                o2.x = pack_bf16(acc.x * inv, acc.y * inv);
+                o2.y = pack_bf16(acc.z * inv, acc.w * inv);
+                const int64_t grow = (int64_t)b.cu_new[s] + tok0 + prow;
+                const int c = pch ^ (prow & (CH - 1));             // un-swizzle: which columns this chunk holds
+                *reinterpret_cast<uint2 *>((char *)a.out + (grow * g.Hq + h) * (D * 2) + c * 8) = o2;
+            }
+        }
+    }
+
+    if (threadIdx.x == 128) TL(33);
     tc_fence_before();
     __syncthreads();
     if (warp == 2)
@@ -467,28 +609,47 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 int sc_tc_tile_m() { return kPairM; }
 int sc_tc_tile_n() { return kTN; }
 
+template <int D>
+static cudaError_t launch_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, dim3 grid, cudaStream_t st)
+{
+    static bool set = false;
+    cudaError_t e;
+    if (!set) {
+        e = cudaFuncSetAttribute(sc_attn_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<D>::kBytes);
+        if (e != cudaSuccess) return e;
+        set = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = Plan<D>::kBytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = a.cluster_combine ? grid.x : 1;       // one CTA per split
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, sc_attn_tc_kernel<D>, g, b, a);
+}
+
+int sc_tc_max_cluster() { return 8; }
+#ifdef SC_TC_PROBE
+extern "C" int sc_probe_read(long long *host) { return (int)cudaMemcpyFromSymbol(host, sc_tl, sizeof(long long) * 256 * 64); }
+#endif
+
 cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st)
 {
     const int total_pairs = b.cu_mt[b.n_seq];
     if (total_pairs == 0) return cudaSuccess;
     dim3 grid((unsigned)a.n_splits, (unsigned)g.Hq, (unsigned)total_pairs);
-    cudaError_t e;
-    if (g.D == 128) {
-        static bool set = false;
-        if (!set) {
-            e = cudaFuncSetAttribute(sc_attn_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<128>::kBytes);
-            if (e != cudaSuccess) return e;
-            set = true;
-        }
-        sc_attn_tc_kernel<128><<<grid, kThreads, Plan<128>::kBytes, st>>>(g, b, a);
-    } else {
-        static bool set = false;
-        if (!set) {
-            e = cudaFuncSetAttribute(sc_attn_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<64>::kBytes);
-            if (e != cudaSuccess) return e;
-            set = true;
-        }
-        sc_attn_tc_kernel<64><<<grid, kThreads, Plan<64>::kBytes, st>>>(g, b, a);
+#ifdef SC_TC_PROBE
+    {
+        const char *pf = getenv("SC_TC_PROBE");
+        const int flags = pf ? atoi(pf) : 0;
+        cudaMemcpyToSymbolAsync(sc_probe_flags, &flags, sizeof flags, 0, cudaMemcpyHostToDevice, st);
     }
-    return cudaGetLastError();
+#endif
+    return g.D == 128 ? launch_tc<128>(g, b, a, grid, st) : launch_tc<64>(g, b, a, grid, st);
 }

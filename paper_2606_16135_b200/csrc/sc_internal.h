@@ -133,6 +133,7 @@ struct ScAttnArgs {
     void *out;          // [sum n][Hq][D] bf16
     ScKvView kv;        // history + new tokens, through the table (or LSC identity)
     float *part_o, *part_ml;
+    int32_t cluster_combine;  // tcgen05 engine: the splits of a query tile group form a cluster and merge in kernel
     int32_t split_tiles;  // KV tiles per split
     int32_t n_splits;     // grid extent over splits (max over rows)
     int32_t total_new;    // sum n
@@ -143,6 +144,7 @@ cudaError_t sc_launch_attn_mma(const ScGeom &g, const ScBatch &b, const ScAttnAr
 // sc_attn_tc.cu  (tcgen05 / TMEM engine): a CTA owns a pair of 128-row query tiles
 int sc_tc_tile_m();
 int sc_tc_tile_n();
+int sc_tc_max_cluster();   // most splits the in-kernel (cluster) combine handles
 cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st);
 cudaError_t sc_launch_combine(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, int tile_m,
                               int tile_n, cudaStream_t st);

@@ -264,6 +264,7 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     a.kv = lv;
     a.part_o = pool->part_o;
     a.part_ml = pool->part_ml;
+    a.cluster_combine = (tc && n_splits > 1 && n_splits <= sc_tc_max_cluster()) ? 1 : 0;
     a.split_tiles = split_tiles;
     a.n_splits = n_splits;
     a.total_new = total_new;
@@ -272,8 +273,9 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
         SC_CUDA(tc ? sc_launch_attn_tc(pool->g, b, a, s) : sc_launch_attn_mma(pool->g, b, a, s));
     }
     pool->launches += 1;
-    // 3. combine (a7)
-    if (n_splits > 1) {
+    // 3. combine (a7): with up to 8 splits the tcgen05 engine merges the partials itself (the
+    //    splits of a query tile group form a thread-block cluster); otherwise a separate kernel
+    if (n_splits > 1 && !a.cluster_combine) {
         {
             ScProfScope ps(pool, SC_KERNEL_COMBINE, s);
             SC_CUDA(sc_launch_combine(pool->g, b, a, tile_m, tile_n, s));
