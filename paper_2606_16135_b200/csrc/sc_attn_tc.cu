@@ -26,6 +26,8 @@
 #include <cuda_bf16.h>
 #include <stdlib.h>
 
+#include <type_traits>
+
 #include "sc_internal.h"
 
 namespace {
@@ -65,6 +67,23 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
             "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return;
+        const long long t = clock64();
+        if (t0 == 0) t0 = t;
+        else if (t - t0 > 4000000000ll) __trap();
+    }
+}
+// same, acquiring at cluster scope (the arrivals come from other CTAs of the cluster)
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    long long t0 = 0;
+    for (;;) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
             "selp.u32 %0, 1, 0, p;\n\t}"
             : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
         if (ok) return;
@@ -183,6 +202,7 @@ struct Bars {                       // at Plan::kBarOff
     uint64_t s_ready[2];            // MMA -> softmax warpgroup m: S_m written (and earlier PV_m done)
     uint64_t p_ready[2];            // softmax warpgroup m -> MMA: P_m stored, O_m rescaled
     uint64_t q_ready[2];            // Q_m in shared memory
+    uint64_t scat_done;             // warps 2-3 -> producer: this CTA's share of the new K/V is in the pool
     uint32_t tmem_base;
 };
 
@@ -192,9 +212,13 @@ __device__ long long sc_tl[256][64];
 #define PROBE(bit) (sc_probe_flags & (1 << (bit)))
 #define TL(i) do { const int cta_ = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z); \
                    if (cta_ < 256) sc_tl[cta_][(i)] = clock64(); } while (0)
+#define TLG(i) do { const int cta_ = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z); \
+                    long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); \
+                    if (cta_ < 256) sc_tl[cta_][(i)] = t_; } while (0)
 #else
 #define PROBE(bit) 0
 #define TL(i) do { } while (0)
+#define TLG(i) do { } while (0)
 #endif
 
 template <int D>
@@ -225,7 +249,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     const int need_max = max(need[0], need[1]);
     const int t_begin = split * a.split_tiles;
     if (t_begin >= need_max) {                   // no keys for this split: only keep the cluster barriers whole
-        if (a.cluster_combine) { cluster_sync_all(); cluster_sync_all(); }
+        if (a.cluster_combine) { cluster_sync_all(); cluster_sync_all(); cluster_sync_all(); }
         return;
     }
     const int t_end = min(t_begin + a.split_tiles, need_max);
@@ -234,10 +258,10 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     for (int m = 0; m < 2; ++m) nt[m] = max(0, min(t_end, need[m]) - t_begin);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x == 0) TL(0);
+    if (threadIdx.x == 0) { TL(0); TLG(60); }
     const uint32_t bar_full = smem_u32(&bars->full[0]), bar_empty = smem_u32(&bars->empty[0]);
     const uint32_t bar_s = smem_u32(&bars->s_ready[0]), bar_p = smem_u32(&bars->p_ready[0]);
-    const uint32_t bar_q = smem_u32(&bars->q_ready[0]);
+    const uint32_t bar_q = smem_u32(&bars->q_ready[0]), bar_scat = smem_u32(&bars->scat_done);
     const uint32_t q_smem = base + P::kQOff, ring = base + P::kRingOff;
 
     if (threadIdx.x == 0) {
@@ -247,6 +271,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             mbar_init(bar_p + 8 * m, kTM);
             mbar_init(bar_q + 8 * m, kTM);
         }
+        mbar_init(bar_scat, a.cluster_combine ? 64 * ((need_max + a.split_tiles - 1) / a.split_tiles) : 256);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
@@ -255,11 +280,82 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
-    __syncthreads();
+    if (a.cluster_combine) cluster_sync_all();      // peers arrive on this CTA's barriers: they must exist
+    else __syncthreads();
     tc_fence_after();
     const uint32_t tmem = bars->tmem_base;
     if (threadIdx.x == 128) TL(1);
     float fin_m = -INFINITY, fin_l = 0.f;      // softmax threads: final (m in log2 units, l) of their row
+
+    // ---- scatter (a5) ----
+    // Without a cluster: the softmax warps do it first; the CTA stores the new tokens at positions [p_lo, p_hi) -- those inside
+    // its own KV tiles that its query tiles can see -- and only relies on its own stores.
+    // With a cluster (one CTA per split of this query pair and head): the pair's new tokens are
+    // dealt out evenly over the cluster's CTAs, whose otherwise idle warps 2-3 store them in the
+    // background, and each thread then arrives (release, cluster
+    // scope) on the scat_done barrier of every CTA of the cluster; a producer waits for all of
+    // them before it loads the first KV tile that holds new tokens.  CTAs of other query heads
+    // of the group or of later query pairs may store the same bytes to the same places.
+    const int ns_act = (need_max + a.split_tiles - 1) / a.split_tiles;        // CTAs of the pair that hold keys
+    auto scatter_share = [&](auto nthreads_c, int tid, auto &&after_first_loads) {
+        constexpr int NT = decltype(nthreads_c)::value;
+        if (a.k_new == nullptr) { after_first_loads(); return; }
+        bool mid_done = false;
+        const int ntok_pair = min(n_s, tok0 + kPairM);
+        int p_lo, ntok, rest_lo, rest_hi;                            // rows of [K rows ; V rows] to store
+        if (a.cluster_combine) {
+            p_lo = T_h; ntok = ntok_pair;
+            const int per = (2 * ntok + ns_act - 1) / ns_act;
+            rest_lo = split * per; rest_hi = min(2 * ntok, rest_lo + per);
+        } else {
+            p_lo = max(T_h, kTN * t_begin); ntok = min(T_h + ntok_pair, kTN * t_end) - p_lo;
+            rest_lo = 0; rest_hi = 2 * ntok;
+        }
+        if (rest_lo < rest_hi) {
+            constexpr int CPR = D / 8;                              // 16-byte units per head row
+            const int hk = h / (g.Hq / g.Hkv);
+            constexpr int RPI = NT / CPR;                           // rows the NT threads cover per step
+            constexpr int U = 8;
+            const int c = tid % CPR;
+            for (int r0 = rest_lo + tid / CPR; r0 < rest_hi; r0 += RPI * U) {
+                int4 val[U];
+#pragma unroll
+                for (int k = 0; k < U; ++k) {
+                    const int rest = r0 + k * RPI;
+                    if (rest < rest_hi) {
+                        const int kv = rest >= ntok, t = rest - kv * ntok;
+                        const int64_t row = (int64_t)b.cu_new[s] + (p_lo + t - T_h);
+                        val[k] = __ldg(reinterpret_cast<const int4 *>(
+                            (const char *)(kv ? a.v_new : a.k_new) + ((row * g.Hkv + hk) * D + c * 8) * 2));
+                    }
+                }
+                if (!mid_done) { after_first_loads(); mid_done = true; }   // overlaps this round trip
+#pragma unroll
+                for (int k = 0; k < U; ++k) {
+                    const int rest = r0 + k * RPI;
+                    if (rest < rest_hi) {
+                        const int kv = rest >= ntok, t = rest - kv * ntok;
+                        const int tok = p_lo + t, lb = tok >> 4, slot = tok & 15;
+                        const int64_t in_cell = (int64_t)(kv * g.Hkv + hk) * P::kChunk + sc_chunk_off(slot, c * 8, NH);
+                        *reinterpret_cast<int4 *>(a.scat0.base + sc_phys_block(a.scat0, b, s, lb) * a.scat0.block_stride + in_cell) = val[k];
+                        if (a.has_scat1)
+                            *reinterpret_cast<int4 *>(a.scat1.base + sc_phys_block(a.scat1, b, s, lb) * a.scat1.block_stride + in_cell) = val[k];
+                    }
+                }
+            }
+            asm volatile("fence.proxy.async.global;" ::: "memory");    // generic-proxy stores before bulk-copy reads
+        }
+        if (!mid_done) after_first_loads();
+        if (a.cluster_combine) {
+            for (int dst = 0; dst < ns_act; ++dst) {
+                uint32_t rbar;
+                asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbar) : "r"(bar_scat), "r"(dst));
+                asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(rbar) : "memory");
+            }
+        } else {
+            mbar_arrive(bar_scat);
+        }
+    };
 
     // registers: the producer / MMA warpgroup gives most of its share to the softmax warpgroups
     if (warp < 4) {
@@ -270,8 +366,14 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             const int nblk = (T_h + n_s + 15) >> 4;
             const int hk = h / (g.Hq / g.Hkv);
             const int64_t off_kv[2] = {(int64_t)hk * P::kChunk, (int64_t)(g.Hkv + hk) * P::kChunk};
+            bool scat_waited = (a.k_new == nullptr);
             for (int jj = 0; jj < nt_max; ++jj) {
                 const int j = t_begin + jj;
+                if (!scat_waited && j >= T_h / kTN) {      // first tile with a block the scatter touches
+                    mbar_wait_cluster(bar_scat, 0);
+                    asm volatile("fence.proxy.async.global;" ::: "memory");   // generic-proxy stores -> bulk-copy reads
+                    scat_waited = true;
+                }
                 const char *blk[8];
 #pragma unroll
                 for (int c = 0; c < 8; ++c) {
@@ -350,6 +452,9 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             }
         }
         __syncwarp();
+    } else if (a.cluster_combine) {
+        // warps 2-3: this CTA's share of the cluster's scatter, in the background
+        scatter_share(std::integral_constant<int, 64>{}, threadIdx.x - 64, []() {});
     }
     } else {
         // =============================== softmax warpgroups ===============================
@@ -359,25 +464,42 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         const int t128 = threadIdx.x - 128 - m * kTM;         // 0..127 inside the warpgroup
         const int row0 = tok0 + m * kTM;                      // first new-token index of the tile
         const int64_t grow = (int64_t)b.cu_new[s] + row0 + r; // packed row of (s, token)
-        if (nt[m] > 0) {
-            // ---- Q_m -> shared memory, swizzled exactly like a K tile ----
+        {
+            // ---- Q_m -> shared memory, swizzled exactly like a K tile; its global loads and the
+            //      first round of scatter loads share one memory round trip ----
             constexpr int CPR = D / 8;                        // 16-byte units per row
             const char *qg = (const char *)a.q;
             const uint32_t qs = q_smem + m * P::kQTile;
+            int4 qv[CPR];
+            if (nt[m] > 0) {
 #pragma unroll
-            for (int it = 0; it < CPR; ++it) {
-                const int u = it * kTM + t128;
-                const int row = u / CPR, c16 = u % CPR, hf = c16 >> 3, c = c16 & 7;
-                int4 v = make_int4(0, 0, 0, 0);
-                if (row < rows[m])
-                    v = __ldg(reinterpret_cast<const int4 *>(
-                        qg + (((int64_t)b.cu_new[s] + row0 + row) * g.Hq + h) * (D * 2) + c16 * 16));
-                const uint32_t dst = qs + (row >> 3) * (NH * 1024) + hf * 1024 + (row & 7) * 128 + ((c ^ (row & 7)) << 4);
-                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" :: "r"(dst), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+                for (int it = 0; it < CPR; ++it) {
+                    const int u = it * kTM + t128;
+                    const int row = u / CPR, c16 = u % CPR;
+                    qv[it] = make_int4(0, 0, 0, 0);
+                    if (row < rows[m])
+                        qv[it] = __ldg(reinterpret_cast<const int4 *>(
+                            qg + (((int64_t)b.cu_new[s] + row0 + row) * g.Hq + h) * (D * 2) + c16 * 16));
+                }
             }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            mbar_arrive(bar_q + 8 * m);
-            if (threadIdx.x == 128) TL(2);
+            auto store_q = [&]() {
+                if (nt[m] > 0) {
+#pragma unroll
+                    for (int it = 0; it < CPR; ++it) {
+                        const int u = it * kTM + t128;
+                        const int row = u / CPR, c16 = u % CPR, hf = c16 >> 3, c = c16 & 7;
+                        const uint32_t dst = qs + (row >> 3) * (NH * 1024) + hf * 1024 + (row & 7) * 128 + ((c ^ (row & 7)) << 4);
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
+                                     :: "r"(dst), "r"(qv[it].x), "r"(qv[it].y), "r"(qv[it].z), "r"(qv[it].w) : "memory");
+                    }
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    mbar_arrive(bar_q + 8 * m);
+                    if (threadIdx.x == 128) TL(2);
+                }
+            };
+            // without a cluster the softmax warps also do the scatter, overlapped with the Q loads
+            if (a.cluster_combine) store_q();
+            else scatter_share(std::integral_constant<int, 256>{}, threadIdx.x - 128, store_q);
         }
 
         const float sl = 1.4426950408889634f * rsqrtf((float)D);      // log2(e)/sqrt(D)
@@ -597,7 +719,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         }
     }
 
-    if (threadIdx.x == 128) TL(33);
+    if (threadIdx.x == 128) { TL(33); TLG(61); }
     tc_fence_before();
     __syncthreads();
     if (warp == 2)

@@ -133,6 +133,10 @@ struct ScAttnArgs {
     void *out;          // [sum n][Hq][D] bf16
     ScKvView kv;        // history + new tokens, through the table (or LSC identity)
     float *part_o, *part_ml;
+    // tcgen05 engine: the scatter of the new K/V (a5) is folded into the attention kernel
+    const void *k_new, *v_new;   // [sum n][Hkv][D] bf16, or nullptr: already scattered
+    ScKvView scat0, scat1;       // where to scatter: the pool, and (staged mode) the LSC
+    int32_t has_scat1;
     int32_t cluster_combine;  // tcgen05 engine: the splits of a query tile group form a cluster and merge in kernel
     int32_t split_tiles;  // KV tiles per split
     int32_t n_splits;     // grid extent over splits (max over rows)

@@ -240,14 +240,7 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     const ScKvView pv = pool_view(pool, layer, tables_dev, max_blocks);
     const ScKvView lv = staged ? lsc_view(pool, buf) : pv;
 
-    // 1. scatter (a5): pool, and the LSC tail in staged mode
-    {
-        ScProfScope ps(pool, SC_KERNEL_SCATTER, s);
-        SC_CUDA(sc_launch_scatter(pool->g, k_new, v_new, b, pv, staged ? &lv : nullptr, s));
-    }
-    pool->launches += 1;
-
-    // 2. attention (a6), split over the keys when that is needed to fill the machine
+    // split of the KV range over CTAs, when that is needed to fill the machine
     int split_tiles = pool->split_tiles_override;
     if (split_tiles <= 0) split_tiles = choose_split_tiles(pool, n_seq, hist_lens, cu_new, tile_m, tile_n, tc ? 1 : 3);
     int max_tiles = 1;
@@ -258,13 +251,30 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
         split_tiles = ceil_div(max_tiles, pool->max_splits);
         n_splits = ceil_div(max_tiles, split_tiles);
     }
+    const bool cluster = tc && n_splits > 1 && n_splits <= sc_tc_max_cluster();
+    // 1. scatter (a5): pool, and the LSC tail in staged mode.  The tcgen05 engine does it inside
+    //    the attention kernel when a query pair's CTAs form a cluster (they share the work) or
+    //    when there is a single CTA per pair; otherwise the scatter kernel runs first.
+    const bool fold_scatter = tc && (cluster || n_splits == 1);
+    if (!fold_scatter) {
+        ScProfScope ps(pool, SC_KERNEL_SCATTER, s);
+        SC_CUDA(sc_launch_scatter(pool->g, k_new, v_new, b, pv, staged ? &lv : nullptr, s));
+        pool->launches += 1;
+    }
+
+    // 2. attention (a6)
     ScAttnArgs a;
     a.q = q;
     a.out = out;
     a.kv = lv;
     a.part_o = pool->part_o;
     a.part_ml = pool->part_ml;
-    a.cluster_combine = (tc && n_splits > 1 && n_splits <= sc_tc_max_cluster()) ? 1 : 0;
+    a.k_new = fold_scatter ? k_new : nullptr;
+    a.v_new = fold_scatter ? v_new : nullptr;
+    a.scat0 = pv;
+    a.scat1 = lv;
+    a.has_scat1 = staged ? 1 : 0;
+    a.cluster_combine = cluster ? 1 : 0;
     a.split_tiles = split_tiles;
     a.n_splits = n_splits;
     a.total_new = total_new;

@@ -47,8 +47,10 @@ class Session:
         self.pool = sc.Pool(self.cfg, self.pool_mem.data_ptr(), pool_bytes,
                             self.lsc_mem.data_ptr() if lsc_blocks else 0, lsc_bytes)
         self.L, self.Hq, self.Hkv, self.D, self.B = L, Hq, Hkv, D, B
-        self.compute_stream = torch.cuda.Stream(device=self.device)
-        self.copy_stream = torch.cuda.Stream(device=self.device)
+        # the compute stream outranks the copy stream: when an SM frees up, an attention CTA (which
+        # needs a whole SM) is placed before the next wave of gather CTAs
+        self.compute_stream = torch.cuda.Stream(device=self.device, priority=-1)
+        self.copy_stream = torch.cuda.Stream(device=self.device, priority=0)
 
     def close(self):
         torch.cuda.synchronize(self.device)
