@@ -680,41 +680,70 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         cluster_sync_all();                  // all partials have landed
         if (threadIdx.x == 128) TL(34);
         if (warp >= 4) {
-            constexpr int RW = 32 / CH;                            // rows a warp handles at once
+            constexpr int RW = 32 / CH;                            // rows a warp handles per step
+            constexpr int RB = 4;                                  // steps in flight
             const int w8 = warp - 4, pch = lane % CH;
             const int r_begin = split * per, n_mine = min(nrows, r_begin + per) - r_begin;
-            for (int i = w8 * RW + lane / CH; i < n_mine; i += 8 * RW) {
-                const int prow = r_begin + i;
-                float2 ml[8];
-                float M = -INFINITY;
+            for (int i0 = w8 * RW + lane / CH; i0 < n_mine; i0 += 8 * RW * RB) {
+                float Mrow[RB];
+                // all loads first (unconditional: a split that sent no O leaves stale but unused bytes)
+                float2 ml[RB][4];
+                float4 v[RB][4];
+                float4 acc[RB];
+                float W[RB];
 #pragma unroll
-                for (int sp = 0; sp < 8; ++sp) {
-                    ml[sp] = make_float2(-INFINITY, 0.f);
-                    if (sp < ns)
-                        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(ml[sp].x), "=f"(ml[sp].y)
-                                     : "r"(recv_ml + (uint32_t)(sp * per + i) * 8));
-                    M = fmaxf(M, ml[sp].x);
-                }
-                float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-                float W = 0.f;
+                for (int k = 0; k < RB; ++k) { acc[k] = make_float4(0.f, 0.f, 0.f, 0.f); W[k] = 0.f; }
 #pragma unroll
-                for (int sp = 0; sp < 8; ++sp) {
-                    const float wgt = (ml[sp].x == -INFINITY) ? 0.f : exp2f(ml[sp].x - M);
-                    if (wgt != 0.f) {                   // an unweighted split sent no O
-                        float4 v;
-                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-                                     : "r"(recv_o + (uint32_t)(sp * per + i) * (D * 4) + pch * 16));
-                        W += wgt * ml[sp].y;
-                        acc.x += wgt * v.x; acc.y += wgt * v.y; acc.z += wgt * v.z; acc.w += wgt * v.w;
+                for (int sp0 = 0; sp0 < 8; sp0 += 4) {          // splits in order, four at a time
+                    if (sp0 >= ns) break;
+#pragma unroll
+                    for (int k = 0; k < RB; ++k) {
+                        const int i = min(i0 + k * 8 * RW, n_mine - 1);   // clamped duplicates are not written
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            const int sp = min(sp0 + q, ns - 1);
+                            asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(ml[k][q].x), "=f"(ml[k][q].y)
+                                         : "r"(recv_ml + (uint32_t)(sp * per + i) * 8));
+                            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                                         : "=f"(v[k][q].x), "=f"(v[k][q].y), "=f"(v[k][q].z), "=f"(v[k][q].w)
+                                         : "r"(recv_o + (uint32_t)(sp * per + i) * (D * 4) + pch * 16));
+                            if (sp0 + q >= ns) ml[k][q] = make_float2(-INFINITY, 0.f);
+                        }
+                    }
+                    // merge this group into the running (M, W, acc) of each row: the running max
+                    // is the first group's max unless a later group raises it (rescale, rare)
+#pragma unroll
+                    for (int k = 0; k < RB; ++k) {
+                        float Mg = fmaxf(fmaxf(ml[k][0].x, ml[k][1].x), fmaxf(ml[k][2].x, ml[k][3].x));
+                        if (sp0 == 0) Mrow[k] = Mg;
+                        else if (Mg > Mrow[k]) {
+                            const float sc = exp2f(Mrow[k] - Mg);   // Mrow finite or -inf (then sc = 0 and acc = 0)
+                            acc[k].x *= sc; acc[k].y *= sc; acc[k].z *= sc; acc[k].w *= sc; W[k] *= sc;
+                            Mrow[k] = Mg;
+                        }
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            const bool on = ml[k][q].x != -INFINITY;
+                            const float wgt = on ? exp2f(ml[k][q].x - Mrow[k]) : 0.f;
+                            W[k] += wgt * ml[k][q].y;
+                            acc[k].x += on ? wgt * v[k][q].x : 0.f; acc[k].y += on ? wgt * v[k][q].y : 0.f;
+                            acc[k].z += on ? wgt * v[k][q].z : 0.f; acc[k].w += on ? wgt * v[k][q].w : 0.f;
+                        }
                     }
                 }
-                const float inv = __fdividef(1.f, W);
-                uint2 o2;
-                o2.x = pack_bf16(acc.x * inv, acc.y * inv);
-                o2.y = pack_bf16(acc.z * inv, acc.w * inv);
-                const int64_t grow = (int64_t)b.cu_new[s] + tok0 + prow;
-                const int c = pch ^ (prow & (CH - 1));             // un-swizzle: which columns this chunk holds
-                *reinterpret_cast<uint2 *>((char *)a.out + (grow * g.Hq + h) * (D * 2) + c * 8) = o2;
+#pragma unroll
+                for (int k = 0; k < RB; ++k) {
+                    const int i = i0 + k * 8 * RW;
+                    if (i >= n_mine) continue;
+                    const int prow = r_begin + i;
+                    const float inv = __fdividef(1.f, W[k]);
+                    uint2 o2;
+                    o2.x = pack_bf16(acc[k].x * inv, acc[k].y * inv);
+                    o2.y = pack_bf16(acc[k].z * inv, acc[k].w * inv);
+                    const int64_t grow = (int64_t)b.cu_new[s] + tok0 + prow;
+                    const int c = pch ^ (prow & (CH - 1));         // un-swizzle: which columns this chunk holds
+                    *reinterpret_cast<uint2 *>((char *)a.out + (grow * g.Hq + h) * (D * 2) + c * 8) = o2;
+                }
             }
         }
     }
