@@ -659,19 +659,43 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" :: "r"(rem_ml), "f"(nt[m] > 0 ? fin_m : -INFINITY),
                              "f"(nt[m] > 0 ? fin_l : 0.f) : "memory");
             if (nt[m] > 0) {
+                // O rows go out through a per-warp 32 x 128-byte transposing scratch (in the idle Q
+                // area), so that a remote store instruction writes four 128-byte runs instead of
+                // 32 isolated 16-byte pieces.  Within a 128-byte run the 16-byte chunks are XORed
+                // with (row & 7) -- conflict-free for the row-per-thread writes, and the same
+                // order in the scratch and at the destination, so the read-out is a linear copy.
                 const uint32_t o_addr = tmem + ((uint32_t)(wl * 32) << 16) + 256 + m * 128;
-                const uint32_t key = (uint32_t)prow & (CH - 1);
+                const uint32_t scratch = q_smem + (uint32_t)(warp - 4) * 4096;
+                uint32_t rem_row[8];                               // destination row of (it*4 + lane/8)
+                bool ok_row[8];
+#pragma unroll
+                for (int it = 0; it < 8; ++it) {
+                    const int pr = m * kTM + wl * 32 + it * 4 + (lane >> 3);
+                    ok_row[it] = pr < nrows;
+                    const int d = ok_row[it] ? pr / per : 0, ii = pr - d * per;
+                    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rem_row[it])
+                                 : "r"(recv_o + (uint32_t)(split * per + ii) * (D * 4) + (lane & 7) * 16), "r"(d));
+                }
 #pragma unroll
                 for (int c4 = 0; c4 < D / 32; ++c4) {
                     uint32_t o[32];
                     tmem_ld32(o_addr + c4 * 32, o);
                     tmem_ld_wait();
-                    if (valid) {
+                    __syncwarp();                                  // previous read-out of the scratch is done
 #pragma unroll
-                        for (int q = 0; q < 8; ++q)
+                    for (int q = 0; q < 8; ++q)
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
+                                     :: "r"(scratch + lane * 128 + (((uint32_t)q ^ (lane & 7)) << 4)), "r"(o[q * 4]), "r"(o[q * 4 + 1]),
+                                        "r"(o[q * 4 + 2]), "r"(o[q * 4 + 3]) : "memory");
+                    __syncwarp();
+#pragma unroll
+                    for (int it = 0; it < 8; ++it) {
+                        uint32_t x, y, z, w;
+                        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(w)
+                                     : "r"(scratch + it * 512 + lane * 16));
+                        if (ok_row[it])
                             asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};"
-                                         :: "r"(rem_o + ((((uint32_t)(c4 * 8 + q)) ^ key) << 4)), "r"(o[q * 4]), "r"(o[q * 4 + 1]),
-                                            "r"(o[q * 4 + 2]), "r"(o[q * 4 + 3]) : "memory");
+                                         :: "r"(rem_row[it] + c4 * 128), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
                     }
                 }
             }
@@ -741,7 +765,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     o2.x = pack_bf16(acc[k].x * inv, acc[k].y * inv);
                     o2.y = pack_bf16(acc[k].z * inv, acc[k].w * inv);
                     const int64_t grow = (int64_t)b.cu_new[s] + tok0 + prow;
-                    const int c = pch ^ (prow & (CH - 1));         // un-swizzle: which columns this chunk holds
+                    const int c = (pch & ~7) | ((pch & 7) ^ (prow & 7));   // un-swizzle: which columns this chunk holds
                     *reinterpret_cast<uint2 *>((char *)a.out + (grow * g.Hq + h) * (D * 2) + c * 8) = o2;
                 }
             }
