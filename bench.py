@@ -127,7 +127,7 @@ class Workload:
         self.hist = list(shape.hist)
         self.n_new = [shape.n_new] * self.n_seq
         self.cu = np.concatenate([[0], np.cumsum(self.n_new)]).astype(np.int32)
-        blocks = [-(-(h + n) // B) for h, n in zip(self.hist, self.n_new)]
+        blocks = [-(-(h + n * shape.turns) // B) for h, n in zip(self.hist, self.n_new)]   # room for every turn
         self.max_blocks = max(blocks)
         pool_kind = sc.SC_POOL_HOST_PINNED if shape.pool_kind == "host" else sc.SC_POOL_HBM
         self.sess = Session(shape.L, shape.Hq, shape.Hkv, shape.D, B, shape.n_blocks, sum(blocks),
@@ -170,6 +170,31 @@ class Workload:
                             sc.SC_MEM_HOST_PINNED if io == "host" else sc.SC_MEM_DEVICE,
                             self.tables_dev.data_ptr(), self.max_blocks, self.hist, self.cu, mode,
                             s.copy_stream.cuda_stream, s.compute_stream.cuda_stream)
+
+    def new_inputs(self, turn: int):
+        """Seeded q / k_new / v_new of all layers for turn `turn` (device)."""
+        I, shape, dev = self.I, self.shape, self.sess.device
+        tot = int(self.cu[-1])
+        self.q = I.normal_bf16_device((shape.L, tot, shape.Hq, shape.D), I.seed_for(shape.config_id, 0, "q", turn=turn), dev)
+        self.k = I.normal_bf16_device((shape.L, tot, shape.Hkv, shape.D), I.seed_for(shape.config_id, 0, "k_new", turn=turn), dev)
+        self.v = I.normal_bf16_device((shape.L, tot, shape.Hkv, shape.D), I.seed_for(shape.config_id, 0, "v_new", turn=turn), dev)
+
+    def advance(self, turn: int):
+        """After a turn: its new tokens are history now (they were scattered into the pool);
+        grow every table for the next turn's new tokens and draw that turn's inputs."""
+        for s in range(self.n_seq):
+            self.hist[s] += self.n_new[s]
+        blocks = [-(-(h + n) // self.shape.B) for h, n in zip(self.hist, self.n_new)]
+        if max(blocks) > self.tables.shape[1]:
+            grown = np.full((self.n_seq, max(blocks) + 64), -1, dtype=np.int32)
+            grown[:, :self.tables.shape[1]] = self.tables
+            self.tables = grown
+        self.max_blocks = self.tables.shape[1]
+        for s in range(self.n_seq):
+            self.n_table[s] = self.sess.pool.append_blocks(self.tables[s], self.n_table[s], self.hist[s], self.n_new[s])
+        self.tables_dev = self.sess.table_dev(self.tables)
+        self.new_inputs(turn)
+        self.torch.cuda.synchronize()
 
     # algorithmic work of one layer (DESIGN.md section 6)
     def layer_flops(self):
@@ -238,6 +263,32 @@ def oracle_sample(w: "Workload", rows=32, budget_s=12.0, max_steps=None):
     return per_layer_s * shape.L * 1e3, info, (a, b, out)
 
 
+# ------------------------------------------------------------------ N > 1: replicas only
+def replica_plan(world: int, rank: int, n_conversations: int = 1) -> dict:
+    """The path has no exchange step: N GPUs run N independent replicas of
+    the workload, each with its own pool and conversations.  Pure bookkeeping, no collective."""
+    return {"replica": rank, "replicas": world, "conversations": n_conversations * world,
+            "collective_on_data_path": None}
+
+
+def max_over_ranks(ms: float, world: int, device="cpu") -> float:
+    """Timing of a multi-rank run is the MAX over ranks (the job is done when the slowest
+    replica is).  Works on any backend (nccl on GPUs, gloo in the CPU tests)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job(ms_per_step: float, world: int, per_replica_kv_bytes: float, per_replica_flops: float) -> dict:
+    """Aggregate throughput of all replicas over the max-over-ranks step time."""
+    return {"kv_gbs": world * per_replica_kv_bytes / ms_per_step / 1e6,
+            "attn_tflops": world * per_replica_flops / ms_per_step / 1e9}
+
+
 # ------------------------------------------------------------------------- ours
 def run_ours(args):
     import torch
@@ -277,12 +328,7 @@ def run_ours(args):
             w.turn(mode, io, bufs)
         ev1.record(xs)
         barrier()
-        ms = ev0.elapsed_time(ev1)
-        if world > 1:
-            t = torch.tensor([ms], device=device)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(ev0.elapsed_time(ev1), world, device)
 
     # warm-up, then the timed region (inputs resident in HBM)
     for _ in range(max(args.warmup, 3)):
@@ -393,6 +439,7 @@ def run_ours(args):
         cpu = {"value": round(cpu_ms, 1), "unit": "ms", **info}
 
     kv_turn_bytes = w.layer_hist_kv_bytes() * shape.L
+    job = whole_job(ms_per_step, world, kv_turn_bytes, w.layer_flops() * shape.L)
     line = {
         "metric": METRIC, "value": round(ms_per_step, 4), "unit": "ms", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": False,
@@ -402,8 +449,8 @@ def run_ours(args):
                                f"{'pinned-host' if shape.pool_kind == 'host' else 'HBM'} pool, {shape.n_new} new tokens",
                    "mode": args.mode, "replicas": world,
                    "l2": f"inputs larger than L2: each turn streams {kv_turn_bytes/1e9:.2f} GB of pool KV"},
-        "kv_gbs": round(world * kv_turn_bytes / ms_per_step / 1e6, 1),
-        "attn_tflops": round(world * w.layer_flops() * shape.L / ms_per_step / 1e9, 1),
+        "kv_gbs": round(job["kv_gbs"], 1),
+        "attn_tflops": round(job["attn_tflops"], 1),
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof, "kernels": kernels,
         "isolated": {k: {"avg_ms": round(avg(v), 5)} for k, v in iso.items() if avg(v) is not None},
