@@ -38,6 +38,10 @@ constexpr int kTN = 128;          // KV tokens per tile (8 pool blocks)
 constexpr int kStages = 5;        // ring slots (each holds the K or the V half of a tile)
 constexpr int kThreads = 384;
 constexpr float kRescaleThreshold = 8.f;   // log2 units
+// Registers.  LEAN = 1 (staged mode): launched with 152 per thread, not the 168 that 384
+// threads could have, so that a 128-thread gather CTA of the copy stream fits beside an
+// attention CTA on the same SM; warps 0-3 then shrink to 56 and the softmax warps grow to 200
+// (setmaxnreg).  LEAN = 0 (fused mode, nothing to share the SM with): 168 -> 72 / 208.
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -221,8 +225,8 @@ __device__ long long sc_tl[256][64];
 #define TLG(i) do { } while (0)
 #endif
 
-template <int D>
-__global__ void __launch_bounds__(kThreads, 1)
+template <int D, int LEAN>
+__global__ void __maxnreg__(LEAN ? 152 : 168)
 sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 {
     using P = Plan<D>;
@@ -315,7 +319,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             constexpr int CPR = D / 8;                              // 16-byte units per head row
             const int hk = h / (g.Hq / g.Hkv);
             constexpr int RPI = NT / CPR;                           // rows the NT threads cover per step
-            constexpr int U = 8;
+            constexpr int U = NT == 64 ? 4 : 8;
             const int c = tid % CPR;
             for (int r0 = rest_lo + tid / CPR; r0 < rest_hi; r0 += RPI * U) {
                 int4 val[U];
@@ -359,7 +363,8 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 
     // registers: the producer / MMA warpgroup gives most of its share to the softmax warpgroups
     if (warp < 4) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
+    if (LEAN) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+    else asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
     if (warp == 0) {
         // =============================== producer ===============================
         if (lane == 0) {
@@ -458,7 +463,8 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     }
     } else {
         // =============================== softmax warpgroups ===============================
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
+        if (LEAN) asm volatile("setmaxnreg.inc.sync.aligned.u32 200;");
+        else asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
         const int m = (warp - 4) >> 2, wl = warp & 3;
         const int r = wl * 32 + lane;                         // row of the query tile = TMEM lane
         const int t128 = threadIdx.x - 128 - m * kTM;         // 0..127 inside the warpgroup
@@ -784,13 +790,13 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 int sc_tc_tile_m() { return kPairM; }
 int sc_tc_tile_n() { return kTN; }
 
-template <int D>
+template <int D, int LEAN>
 static cudaError_t launch_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, dim3 grid, cudaStream_t st)
 {
     static bool set = false;
     cudaError_t e;
     if (!set) {
-        e = cudaFuncSetAttribute(sc_attn_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<D>::kBytes);
+        e = cudaFuncSetAttribute(sc_attn_tc_kernel<D, LEAN>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<D>::kBytes);
         if (e != cudaSuccess) return e;
         set = true;
     }
@@ -806,7 +812,7 @@ static cudaError_t launch_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, sc_attn_tc_kernel<D>, g, b, a);
+    return cudaLaunchKernelEx(&cfg, sc_attn_tc_kernel<D, LEAN>, g, b, a);
 }
 
 int sc_tc_max_cluster() { return 8; }
@@ -826,5 +832,7 @@ cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArg
         cudaMemcpyToSymbolAsync(sc_probe_flags, &flags, sizeof flags, 0, cudaMemcpyHostToDevice, st);
     }
 #endif
-    return g.D == 128 ? launch_tc<128>(g, b, a, grid, st) : launch_tc<64>(g, b, a, grid, st);
+    if (a.has_scat1)   // staged mode: a gather runs beside this kernel
+        return g.D == 128 ? launch_tc<128, 1>(g, b, a, grid, st) : launch_tc<64, 1>(g, b, a, grid, st);
+    return g.D == 128 ? launch_tc<128, 0>(g, b, a, grid, st) : launch_tc<64, 0>(g, b, a, grid, st);
 }

@@ -7,6 +7,8 @@
 // 16-byte vectors, coalesced, several independent requests in flight per thread; the
 // bulk variant moves whole pieces with the TMA engine (cp.async.bulk) through a
 // shared-memory ring and keeps the SM's LSU out of it.
+#include <stdlib.h>
+
 #include "sc_internal.h"
 
 namespace {
@@ -67,9 +69,9 @@ sc_scatter_read_kernel(ScGeom g, ScBatch b, char *k_lin, char *v_lin, ScKvView v
 }
 
 // ------------------------------------------------------------ gather (LDG/STG)
-constexpr int kGatherThreads = 256;
+constexpr int kGatherThreads = 128;   // small CTAs: one fits beside a tcgen05 attention CTA (registers)
 constexpr int kGatherUnroll = 8;
-constexpr int kGatherPiece = kGatherThreads * 16 * kGatherUnroll;   // 32 KiB per CTA
+constexpr int kGatherPiece = kGatherThreads * 16 * kGatherUnroll;   // 16 KiB per CTA
 
 __global__ void __launch_bounds__(kGatherThreads)
 sc_gather_ldg_kernel(ScGeom g, ScBatch b, ScKvView src, ScKvView dst, int pieces_per_cell)
@@ -227,6 +229,9 @@ cudaError_t sc_launch_gather(const ScGeom &g, const ScBatch &b, const ScKvView &
                 attr_set = true;
             }
             int grid = n_sms < n_items ? n_sms : n_items;
+#ifdef SC_TC_PROBE
+            if (const char *e = getenv("SC_BULK_GRID")) grid = atoi(e) < n_items ? atoi(e) : n_items;
+#endif
             sc_gather_bulk_kernel<<<grid, 32, smem, st>>>(g, b, src, dst, ppc, piece, n_items);
             return cudaGetLastError();
         }
