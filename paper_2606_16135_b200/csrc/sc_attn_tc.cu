@@ -395,6 +395,14 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     for (int c = 0; c < 8; ++c)
                         bulk_g2s(ring + slot * P::kSlot + c * P::kChunk, blk[c] + off_kv[kv], P::kChunk,
                                  bar_full + 8 * slot);
+                    if (it == 0) {
+                        // The first MMA needs Q and K of tile 0 only.  All CTAs start together, so
+                        // the rest of the ring is requested once Q has landed: it would only queue
+                        // in front of Q at the memory controllers.
+#pragma unroll
+                        for (int m = 0; m < 2; ++m)
+                            if (nt[m] > 0) mbar_wait(bar_q + 8 * m, 0);
+                    }
                 }
             }
         }
