@@ -37,6 +37,7 @@ constexpr int kPairM = 2 * kTM;   // rows a CTA owns
 constexpr int kTN = 128;          // KV tokens per tile (8 pool blocks)
 constexpr int kStages = 5;        // ring slots (each holds the K or the V half of a tile)
 constexpr int kThreads = 384;
+constexpr int kMaxCluster = 16;   // most splits merged in kernel (non-portable cluster size)
 constexpr float kRescaleThreshold = 8.f;   // log2 units
 // Registers.  LEAN = 1 (staged mode): launched with 152 per thread, not the 168 that 384
 // threads could have, so that a 128-thread gather CTA of the copy stream fits beside an
@@ -657,7 +658,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         const int ns = (need_max + a.split_tiles - 1) / a.split_tiles;     // CTAs that hold keys
         const int nrows = min(kPairM, n_s - tok0);
         const int per = (nrows + ns - 1) / ns;                     // rows per CTA
-        const uint32_t recv_o = ring, recv_ml = ring + (kPairM + 8) * D * 4;   // [src][per][D] fp32, [src][per] (m, l)
+        const uint32_t recv_o = ring, recv_ml = ring + (kPairM + 16) * D * 4;   // [src][per][D] fp32, [src][per] (m, l)
         cluster_sync_all();                  // every CTA of the cluster is done with its ring
         if (threadIdx.x == 128) TL(31);
         if (warp >= 4) {
@@ -732,7 +733,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 #pragma unroll
                 for (int k = 0; k < RB; ++k) { acc[k] = make_float4(0.f, 0.f, 0.f, 0.f); W[k] = 0.f; }
 #pragma unroll
-                for (int sp0 = 0; sp0 < 8; sp0 += 4) {          // splits in order, four at a time
+                for (int sp0 = 0; sp0 < kMaxCluster; sp0 += 4) { // splits in order, four at a time
                     if (sp0 >= ns) break;
 #pragma unroll
                     for (int k = 0; k < RB; ++k) {
@@ -799,31 +800,71 @@ int sc_tc_tile_m() { return kPairM; }
 int sc_tc_tile_n() { return kTN; }
 
 template <int D, int LEAN>
-static cudaError_t launch_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, dim3 grid, cudaStream_t st)
+static cudaError_t prepare_tc()
 {
     static bool set = false;
-    cudaError_t e;
-    if (!set) {
-        e = cudaFuncSetAttribute(sc_attn_tc_kernel<D, LEAN>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<D>::kBytes);
-        if (e != cudaSuccess) return e;
-        set = true;
-    }
-    cudaLaunchConfig_t cfg = {};
+    if (set) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(sc_attn_tc_kernel<D, LEAN>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<D>::kBytes);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(sc_attn_tc_kernel<D, LEAN>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    set = (e == cudaSuccess);
+    return e;
+}
+
+template <int D, int LEAN>
+static void fill_config(cudaLaunchConfig_t &cfg, cudaLaunchAttribute *attr, dim3 grid, int cluster, cudaStream_t st)
+{
+    cfg = cudaLaunchConfig_t{};
     cfg.gridDim = grid;
     cfg.blockDim = dim3(kThreads);
     cfg.dynamicSmemBytes = Plan<D>::kBytes;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = a.cluster_combine ? grid.x : 1;       // one CTA per split
+    attr[0].val.clusterDim.x = cluster;                               // one CTA per split
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+}
+
+template <int D, int LEAN>
+static cudaError_t launch_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, dim3 grid, cudaStream_t st)
+{
+    cudaError_t e = prepare_tc<D, LEAN>();
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    fill_config<D, LEAN>(cfg, attr, grid, a.cluster_combine ? (int)grid.x : 1, st);
     return cudaLaunchKernelEx(&cfg, sc_attn_tc_kernel<D, LEAN>, g, b, a);
 }
 
-int sc_tc_max_cluster() { return 8; }
+// CTAs that can be resident at once when the kernel is launched in clusters of `cluster` CTAs
+// (each CTA needs a whole SM; a cluster must fit in one GPC).  0 if such clusters cannot launch.
+template <int D, int LEAN>
+static int wave_ctas(int cluster)
+{
+    if (prepare_tc<D, LEAN>() != cudaSuccess) return 0;
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    fill_config<D, LEAN>(cfg, attr, dim3((unsigned)cluster, 1, 1), cluster, nullptr);
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, sc_attn_tc_kernel<D, LEAN>, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return n * cluster;
+}
+
+int sc_tc_max_cluster() { return kMaxCluster; }
+
+int sc_tc_wave_ctas(int D, int lean, int cluster)
+{
+    static int cache[2][2][kMaxCluster + 1];                          // 0 = not asked yet, -1 = cannot launch
+    int &c = cache[D == 128][lean != 0][cluster];
+    if (c == 0) {
+        const int n = D == 128 ? (lean ? wave_ctas<128, 1>(cluster) : wave_ctas<128, 0>(cluster))
+                               : (lean ? wave_ctas<64, 1>(cluster) : wave_ctas<64, 0>(cluster));
+        c = n > 0 ? n : -1;
+    }
+    return c > 0 ? c : 0;
+}
 #ifdef SC_TC_PROBE
 extern "C" int sc_probe_read(long long *host) { return (int)cudaMemcpyFromSymbol(host, sc_tl, sizeof(long long) * 256 * 64); }
 #endif

@@ -149,6 +149,7 @@ cudaError_t sc_launch_attn_mma(const ScGeom &g, const ScBatch &b, const ScAttnAr
 int sc_tc_tile_m();
 int sc_tc_tile_n();
 int sc_tc_max_cluster();   // most splits the in-kernel (cluster) combine handles
+int sc_tc_wave_ctas(int D, int lean, int cluster);   // co-resident CTAs when launched in clusters of that size
 cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st);
 cudaError_t sc_launch_combine(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, int tile_m,
                               int tile_n, cudaStream_t st);

@@ -1,5 +1,7 @@
 // sc_ops.cu -- the data calls of the C ABI (a3-a9): argument checking on the host,
 // then kernel launches on the caller's stream.  No step of the path runs on the CPU.
+#include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -86,15 +88,23 @@ int lsc_blocks_needed(const ScBatch &b) { return b.lsc_total; }
 // `split` tiles each; the grid runs in waves of n_sms*ctas_per_sm CTAs, and a CTA costs its
 // tiles plus a fixed overhead (prologue, epilogue, partial write + combine read).  Pick the
 // split with the smallest  waves * (split + overhead).  Depends on logical lengths only.
-int choose_split_tiles(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, const int32_t *cu_new,
-                       int tile_m, int tile_n, int ctas_per_sm)
+// KV tiles per split, and whether the splits of a query pair run as one thread-block cluster.
+// Every (query tile group, head) needs ceil(tiles/split) CTAs of up to `split` tiles each; the
+// grid runs in waves, and a CTA costs its tiles plus a fixed overhead (prologue, epilogue).
+// Costs are in units of one KV tile (~1.9 us on B200), fitted to measurements:
+//   cluster (tcgen05, <= 16 splits, ONE wave only -- clusters of whole-SM CTAs place badly over
+//            several waves -- and <= 128 tiles per CTA): in-kernel scatter + DSMEM combine, ~4
+//   plain  : separate scatter (~5) and combine (~1.3 per split) kernels, partial write ~2 per wave
+// Depends on logical lengths only.
+struct SplitChoice { int split_tiles; bool cluster; };
+
+SplitChoice choose_split_tiles(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, const int32_t *cu_new,
+                               int tile_m, int tile_n, bool tc, bool staged)
 {
     int max_tiles = 1;
     for (int i = 0; i < n_seq; ++i)
         max_tiles = std::max(max_tiles, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), tile_n));
-    const int64_t wave = (int64_t)p->n_sms * ctas_per_sm;
-    const double overhead = 2.5;
-    int best = max_tiles;
+    SplitChoice best = {max_tiles, false};
     double best_cost = 1e30;
     for (int n_sp = 1; n_sp <= p->max_splits; ++n_sp) {
         const int split = ceil_div(max_tiles, n_sp);
@@ -107,11 +117,30 @@ int choose_split_tiles(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, 
                 ctas += (int64_t)p->g.Hq * ceil_div(ceil_div(kmax, tile_n), split);
             }
         }
-        const double waves = (double)((ctas + wave - 1) / wave);
-        const double cost = waves * (split + overhead) + (n_sp > 1 ? 0.5 : 0.0);
-        if (cost < best_cost - 1e-9) { best_cost = cost; best = split; }
+        for (int use_cluster = 0; use_cluster < 2; ++use_cluster) {
+            int64_t wave = (int64_t)p->n_sms * (tc ? 1 : 3);
+            double extra = 0.0;
+            if (use_cluster) {
+                if (!tc || n_sp < 2 || n_sp > sc_tc_max_cluster() || split > 128) continue;
+                wave = sc_tc_wave_ctas(p->g.D, staged, n_sp);
+                // the launch is n_sp CTAs per (pair, head) whether or not a sequence needs them all
+                int64_t launched = 0;
+                for (int i = 0; i < n_seq; ++i)
+                    launched += (int64_t)p->g.Hq * ceil_div(cu_new[i + 1] - cu_new[i], tile_m) * n_sp;
+                if (wave <= 0 || launched > wave) continue;
+                extra = 4.0;
+            }
+            const double waves = (double)((ctas + wave - 1) / wave);
+            if (!use_cluster && n_sp > 1) extra = (tc ? 5.0 : 0.5) + 1.3 * n_sp + 2.0 * waves;
+            const double cost = waves * (split + 3.0) + extra;
+#ifdef SC_TC_PROBE
+            if (getenv("SC_DEBUG_SPLIT")) fprintf(stderr, "n_sp %d cluster %d split %d ctas %lld wave %lld waves %.0f cost %.1f\n", n_sp, use_cluster, split, (long long)ctas, (long long)wave, waves, cost);
+#endif
+            if (cost < best_cost - 1e-9) { best_cost = cost; best = {split, use_cluster != 0}; }
+        }
     }
-    return std::max(best, 1);
+    best.split_tiles = std::max(best.split_tiles, 1);
+    return best;
 }
 
 }  // namespace
@@ -242,16 +271,26 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
 
     // split of the KV range over CTAs, when that is needed to fill the machine
     int split_tiles = pool->split_tiles_override;
-    if (split_tiles <= 0) split_tiles = choose_split_tiles(pool, n_seq, hist_lens, cu_new, tile_m, tile_n, tc ? 1 : 3);
+    bool cluster = false;
     int max_tiles = 1;
     for (int i = 0; i < n_seq; ++i)
         max_tiles = std::max(max_tiles, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), tile_n));
+    if (split_tiles <= 0) {
+        const SplitChoice c = choose_split_tiles(pool, n_seq, hist_lens, cu_new, tile_m, tile_n, tc, staged);
+        split_tiles = c.split_tiles;
+        cluster = c.cluster;
+    } else {
+        // forced split (tests, experiments): cluster whenever such a cluster can be placed
+        const int ns = ceil_div(max_tiles, split_tiles);
+        cluster = tc && ns > 1 && ns <= sc_tc_max_cluster() && sc_tc_wave_ctas(pool->g.D, staged, ns) > 0;
+    }
     int n_splits = ceil_div(max_tiles, split_tiles);
     if (n_splits > pool->max_splits) {
         split_tiles = ceil_div(max_tiles, pool->max_splits);
         n_splits = ceil_div(max_tiles, split_tiles);
+        cluster = false;
     }
-    const bool cluster = tc && n_splits > 1 && n_splits <= sc_tc_max_cluster();
+    if (n_splits == 1) cluster = false;
     // 1. scatter (a5): pool, and the LSC tail in staged mode.  The tcgen05 engine does it inside
     //    the attention kernel when a query pair's CTAs form a cluster (they share the work) or
     //    when there is a single CTA per pair; otherwise the scatter kernel runs first.
