@@ -177,6 +177,29 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
+// ---- packed fp32x2 arithmetic (FFMA2 / FADD2 on sm_100): halves the FMA-pipe instructions of the softmax ----
+__device__ __forceinline__ uint64_t pk2(float lo, float hi)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk2(uint64_t v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c)
+{
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b)
+{
+    uint64_t d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
 {
     __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
@@ -573,15 +596,28 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 }
             }
             const float msl = (m_used == -INFINITY) ? 0.f : m_used * sl;
-            float rs4[4] = {0.f, 0.f, 0.f, 0.f};
+            // P = 2^(s*sl - m*sl), two columns at a time.  (Moving a share of the exp2 to the FMA pipe
+            // with a polynomial was measured slower at every share: with one softmax warp per
+            // scheduler and query tile the loop is issue-bound, not MUFU-bound.)
+            const uint64_t sl2 = pk2(sl, sl), nmsl2 = pk2(-msl, -msl);
+            uint64_t rs2[2] = {0ull, 0ull};                     // (0.f, 0.f)
 #pragma unroll
             for (int c = 0; c < kTN / 2; ++c) {
-                const float p0 = exp2f(fmaf(__uint_as_float(sv[2 * c]), sl, -msl));
-                const float p1 = exp2f(fmaf(__uint_as_float(sv[2 * c + 1]), sl, -msl));
-                rs4[c & 3] += p0 + p1;
+                uint64_t x = fma2(pk2(__uint_as_float(sv[2 * c]), __uint_as_float(sv[2 * c + 1])), sl2, nmsl2);
+                float p0, p1;
+                upk2(x, p0, p1);
+                p0 = exp2f(p0);
+                p1 = exp2f(p1);
+                x = pk2(p0, p1);
+                rs2[c & 1] = add2(rs2[c & 1], x);
                 sv[c] = pack_bf16(p0, p1);                      // in place: c <= 2c
             }
-            l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
+            {
+                float a0, a1, b0, b1;
+                upk2(rs2[0], a0, a1);
+                upk2(rs2[1], b0, b1);
+                l_run += (a0 + a1) + (b0 + b1);
+            }
             tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&sv[0]));
             tmem_st32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[32]));
             tmem_st_wait();
