@@ -12,13 +12,19 @@
 //   warp 1      MMA      : one thread issues tcgen05.mma.  S_m = Q_m K^T (both operands in
 //                          shared memory, K-major) into TMEM; O_m += P_m V with P_m read from
 //                          TMEM and V as an MN-major shared-memory operand.
-//   warp 2      TMEM allocation (all 512 columns: S0 S1 O0 O1, 128 fp32 columns each)
+//   warp 2      TMEM allocation (all 512 columns: S0 S1 O0 O1, 128 fp32 columns each);
+//   warps 2-3   in cluster mode: this CTA's share of the scatter of the new K/V (a5)
 //   warps 4-7   softmax warpgroup of query tile 0: thread r owns row r.  tcgen05.ld S,
 //   warps 8-11  same for query tile 1            : mask, online softmax in registers with
 //                          lazy rescaling of O (only when the row max grows by > 2^8), P
 //                          rounded to bf16 and stored over S in TMEM, epilogue.
 // The two query tiles ping-pong on the tensor pipe: while warpgroup 0 does the softmax of
 // tile j, the pipe runs PV and QK^T of query tile 1.
+//
+// Split-KV (a7): with up to 16 splits that fit one wave, the CTAs of one (query pair, head) are
+// a thread-block cluster; they share the scatter and merge their partial (m, l, O) through
+// distributed shared memory at the end.  Otherwise partials go to global scratch and
+// sc_combine_kernel merges them, and the scatter kernel runs before this one.
 //
 // Work partitioning depends on logical positions only, so results are bit-identical under
 // any permutation of physical block ids, and staged attention is this same kernel run with
