@@ -189,3 +189,39 @@ def test_host_pinned_pool_matches_oracle():
     off = p.cell_offset(int(cv.tables[0][t // 16]), 1, 0, h, t % 16, d)
     assert raw[off // 2] == cv.logical[0][1][0][t, h, d]
     cv.sess.close()
+
+
+@pytest.mark.parametrize("slow", ["copy", "compute"])
+def test_pipeline_ordering_survives_a_slow_stream(slow):
+    """PAPER.md:192 ordering rule (reading S8): attention(l) must wait for load(l), load(l+1) for
+    attention(l-1).  One of the two streams is held up by a long busy kernel right before the
+    turns are enqueued; if an event were missing, the other stream would run ahead and read an
+    LSC buffer that is not loaded yet (or overwrite one that is still being read)."""
+    cv = Conversations(L=6, Hq=4, Hkv=4, D=128, hist=[1500, 300], NB=260, max_new=200, seed=17)
+    p, dev = cv.sess.pool, cv.sess.device
+    refs, outs, keep = [], [], []
+    for turn in range(2):
+        n_new = [100, 37]
+        cv.begin_turn(n_new)
+        q_all, k_all, v_all = cv.make_inputs(n_new, 700 + turn)
+        refs.append(cv.oracle_turn(q_all, k_all, v_all))
+        tq, tk, tv = (bits_to_torch(x, dev) for x in (q_all, k_all, v_all))
+        out = torch.zeros_like(tq)
+        torch.cuda.synchronize()
+        keep.append((tq, tk, tv))
+        stream = cv.sess.copy_stream if slow == "copy" else cv.sess.compute_stream
+        with torch.cuda.stream(stream):
+            torch.cuda._sleep(int(2e8))                    # ~0.1 s of busy waiting on that stream
+        p.prefill_turn(tq.data_ptr(), tk.data_ptr(), tv.data_ptr(), out.data_ptr(), sc.SC_MEM_DEVICE,
+                       cv.tables_dev.data_ptr(), cv.max_blocks, cv.hist, cv.cu, sc.SC_ATTN_STAGED,
+                       cv.sess.copy_stream.cuda_stream, cv.sess.compute_stream.cuda_stream)
+        outs.append(out)
+        cv.end_turn(n_new)
+        torch.cuda.current_stream().wait_stream(cv.sess.compute_stream)
+        torch.cuda.current_stream().wait_stream(cv.sess.copy_stream)
+    torch.cuda.synchronize()
+    for turn in range(2):
+        for l in range(cv.L):
+            assert_close(torch_to_bits(outs[turn][l]), refs[turn][l], f"slow {slow}: turn {turn} layer {l}")
+    cv.check_pool_equals_logical()
+    cv.sess.close()
