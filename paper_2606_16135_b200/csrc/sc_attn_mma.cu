@@ -308,11 +308,10 @@ cudaError_t sc_launch_attn_mma(const ScGeom &g, const ScBatch &b, const ScAttnAr
     cudaError_t e;
     if (g.D == 128) {
         constexpr int smem = 2 * 8 * 16 * 128 * 2;
-        static bool set = false;
-        if (!set) {
+        static std::atomic<uint64_t> done{0};
+        if (sc_first_use_on_device(done)) {
             e = cudaFuncSetAttribute(sc_attn_mma_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
             if (e != cudaSuccess) return e;
-            set = true;
         }
         sc_attn_mma_kernel<128><<<grid, kThreads, smem, st>>>(g, b, a);
     } else {

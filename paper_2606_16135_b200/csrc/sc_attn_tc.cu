@@ -844,12 +844,11 @@ int sc_tc_tile_n() { return kTN; }
 template <int D, int LEAN>
 static cudaError_t prepare_tc()
 {
-    static bool set = false;
-    if (set) return cudaSuccess;
+    static std::atomic<uint64_t> done{0};
+    if (!sc_first_use_on_device(done)) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute(sc_attn_tc_kernel<D, LEAN>, cudaFuncAttributeMaxDynamicSharedMemorySize, Plan<D>::kBytes);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(sc_attn_tc_kernel<D, LEAN>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-    set = (e == cudaSuccess);
     return e;
 }
 
@@ -898,8 +897,10 @@ int sc_tc_max_cluster() { return kMaxCluster; }
 
 int sc_tc_wave_ctas(int D, int lean, int cluster)
 {
-    static int cache[2][2][kMaxCluster + 1];                          // 0 = not asked yet, -1 = cannot launch
-    int &c = cache[D == 128][lean != 0][cluster];
+    static int cache[SC_MAX_DEVICES][2][2][kMaxCluster + 1];          // 0 = not asked yet, -1 = cannot launch
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= SC_MAX_DEVICES) dev = 0;
+    int &c = cache[dev][D == 128][lean != 0][cluster];
     if (c == 0) {
         const int n = D == 128 ? (lean ? wave_ctas<128, 1>(cluster) : wave_ctas<128, 0>(cluster))
                                : (lean ? wave_ctas<64, 1>(cluster) : wave_ctas<64, 0>(cluster));

@@ -220,13 +220,12 @@ cudaError_t sc_launch_gather(const ScGeom &g, const ScBatch &b, const ScKvView &
         const int ppc = (int)(g.cell_bytes / piece);     // cell_bytes is a multiple of 4 KiB
         if ((int64_t)ppc * piece == g.cell_bytes) {
             const int n_items = total_blocks * ppc;
-            static bool attr_set = false;
+            static std::atomic<uint64_t> done{0};
             const int smem = kBulkStages * kBulkPiece;
-            if (!attr_set) {
+            if (sc_first_use_on_device(done)) {
                 cudaError_t e = cudaFuncSetAttribute(sc_gather_bulk_kernel,
                                                      cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
                 if (e != cudaSuccess) return e;
-                attr_set = true;
             }
             int grid = n_sms < n_items ? n_sms : n_items;
 #ifdef SC_TC_PROBE

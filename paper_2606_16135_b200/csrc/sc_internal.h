@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <mutex>
 #include <vector>
 
@@ -117,6 +118,17 @@ struct ScProfScope {
 sc_status_t sc_fail(sc_status_t code, const char *fmt, ...);
 sc_status_t sc_cuda_fail(cudaError_t e, const char *what);
 const char *sc_err_buf();
+
+// Function attributes (dynamic shared memory, cluster size) are per device: true the first
+// time it is called for the calling thread's current device with this mask (up to 64 devices).
+inline bool sc_first_use_on_device(std::atomic<uint64_t> &mask)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev > 63) return true;   // just set it again
+    const uint64_t bit = 1ull << dev;
+    return (mask.fetch_or(bit) & bit) == 0;
+}
+constexpr int SC_MAX_DEVICES = 64;
 
 // ------------------------------------------------------- kernel launchers
 // sc_copy.cu
