@@ -341,6 +341,16 @@ def run_ours(args):
     clocks = clk.stop() if clk else None
     ms_per_step = total_ms / args.steps
 
+    # the other variant of the path beside it (same workload, same timing protocol, fewer steps):
+    # fused = attention reads pool blocks through the block table, no gather into the LSC
+    other_mode = sc.SC_ATTN_FUSED if mode == sc.SC_ATTN_STAGED else sc.SC_ATTN_STAGED
+    saved_mode, mode = mode, other_mode
+    for _ in range(3):
+        w.turn(mode)
+    o_steps = max(3, min(args.steps, 50))
+    other_ms = timed(o_steps) / o_steps
+    mode = saved_mode
+
     # end to end through the C ABI with HOST buffers (pinned): H2D of q/k/v and D2H of out inside
     e2e = None
     if not args.no_e2e:
@@ -451,6 +461,8 @@ def run_ours(args):
                    "l2": f"inputs larger than L2: each turn streams {kv_turn_bytes/1e9:.2f} GB of pool KV"},
         "kv_gbs": round(job["kv_gbs"], 1),
         "attn_tflops": round(job["attn_tflops"], 1),
+        "other_mode": {"mode": "fused" if other_mode == sc.SC_ATTN_FUSED else "staged", "value": round(other_ms, 4),
+                       "unit": "ms", "steps": o_steps},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof, "kernels": kernels,
         "isolated": {k: {"avg_ms": round(avg(v), 5)} for k, v in iso.items() if avg(v) is not None},
