@@ -22,6 +22,8 @@
  *                       softmax scale 1/sqrt(D) (reading S1 in DESIGN.md)
  *   O5  append count    ceil((T_h+n)/B) - ceil(T_h/B) new table entries
  *                       (PAPER.md:142 block table; reading S10)
+ *   O7  sizing          K_i, K_master, N_LSC, N_RC (Eq. 2-5); MEU / LCM
+ *                       (Eq. 6-9); ScaleUp / ScaleDown (Algorithm 1)
  *
  * Precision: the north star fixes the oracle at fp32 ("a plain, slow CPU
  * fp32 implementation"); sco_attention_f64 is the same algorithm in double,
@@ -224,6 +226,73 @@ int sco_softmax_row_f32(const uint16_t *q, const uint16_t *K, int32_t T_h, int32
     for (int32_t j = 0; j < nk; ++j) { p_out[j] = expf(p_out[j] - m); denom += p_out[j]; }
     for (int32_t j = 0; j < nk; ++j) p_out[j] /= denom;
     return 0;
+}
+
+/* ---------------------------------------------------- sizing and elasticity -- */
+/* Host integer arithmetic of Sec. 3.2 and 3.4-3.5, written out
+ * as printed.  Pins: the worked example of PAPER.md:180 (tests/golden), lcm identities checked
+ * against a brute-force search, hand-computed Algorithm 1 cases.                             */
+
+/* Eq. 2-5 (the printed |.| of Eq. 2 and 5 are floors, reading S11).
+ * c_master, c_worker[i]: KV cache bytes; m_block: Eq. 1; L: master layers.
+ * out[0] = K_master (Eq. 3), out[1] = sum_i K_i (Eq. 2), out[2] = N_LSC (Eq. 4),
+ * out[3] = N_RC (Eq. 5), out[4] = (N_LSC + N_RC) * 1 blocks = max context in blocks,
+ * out[5] = floor(K_master / L): what a conventional full-layer cache holds.              */
+int sco_lsc_rc_sizing(int64_t c_master, const int64_t *c_worker, int32_t n_workers,
+                      int64_t m_block, int32_t L, int64_t *out)
+{
+    if (c_master < 0 || n_workers < 0 || m_block <= 0 || L <= 0) return -1;
+    int64_t k_master = c_master / m_block;                       /* Eq. 3 */
+    int64_t sum_k = 0;
+    for (int32_t i = 0; i < n_workers; ++i) {
+        if (c_worker[i] < 0) return -1;
+        sum_k += c_worker[i] / (m_block * L);                    /* Eq. 2 */
+    }
+    int64_t n_lsc = sum_k < k_master ? sum_k : k_master;         /* Eq. 4 */
+    int64_t n_rc = sum_k < k_master ? (k_master - sum_k) / L : 0;   /* Eq. 5 */
+    out[0] = k_master; out[1] = sum_k; out[2] = n_lsc; out[3] = n_rc;
+    out[4] = n_lsc + n_rc; out[5] = k_master / L;
+    return 0;
+}
+
+/* Eq. 6-9: BE = L*B*Hkv*Dkv elements of one full-layer block;
+ * LCM_elem = lcm(BE_m, BE_i); MEU_m = LCM/BE_m, MEU_i = LCM/BE_i.                        */
+int64_t sco_block_elems(int32_t L, int32_t B, int32_t Hkv, int32_t D)
+{
+    return (int64_t)L * B * Hkv * D;
+}
+
+int sco_meu(int64_t be_m, int64_t be_i, int64_t *meu_m, int64_t *meu_i)
+{
+    if (be_m <= 0 || be_i <= 0) return -1;
+    int64_t a = be_m, b = be_i;
+    while (b) { int64_t t = a % b; a = b; b = t; }               /* a = gcd */
+    int64_t lcm = be_m / a * be_i;                               /* Eq. 8 */
+    *meu_m = lcm / be_m;                                         /* Eq. 9 */
+    *meu_i = lcm / be_i;
+    return 0;
+}
+
+/* Algorithm 1, ScaleUp: blocks the i-th worker gains and the master gives up. */
+void sco_scale_up(int64_t n_i, int64_t b_i, int64_t meu_i, int64_t meu_m, int64_t request_len,
+                  int64_t *d_worker, int64_t *d_master)
+{
+    int64_t need = (request_len + b_i - 1) / b_i;
+    if (need <= n_i) { *d_worker = 0; *d_master = 0; return; }
+    int64_t diff = need - n_i;
+    int64_t k = (diff + meu_i - 1) / meu_i;
+    *d_worker = k * meu_i; *d_master = k * meu_m;
+}
+
+/* Algorithm 1, ScaleDown: max_len = longest request of the last t seconds. */
+void sco_scale_down(int64_t n_i, int64_t b_i, int64_t meu_i, int64_t meu_m, int64_t max_len,
+                    int64_t *d_worker, int64_t *d_master)
+{
+    int64_t max_need = (max_len + b_i - 1) / b_i;
+    if (max_need >= n_i) { *d_worker = 0; *d_master = 0; return; }
+    int64_t diff = n_i - max_need;
+    int64_t k = diff / meu_i;
+    *d_worker = k * meu_i; *d_master = k * meu_m;
 }
 
 int sco_openmp_threads(void)

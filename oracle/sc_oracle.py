@@ -59,6 +59,15 @@ def _load():
         lib.sco_attention_f32.argtypes = common + [f32p, f32p]
         lib.sco_attention_f64.argtypes = common + [f64p, f64p]
         lib.sco_softmax_row_f32.argtypes = [u16p, u16p] + [C.c_int32] * 6 + [f32p]
+        i64p = C.POINTER(C.c_int64)
+        lib.sco_lsc_rc_sizing.argtypes = [C.c_int64, i64p, C.c_int32, C.c_int64, C.c_int32, i64p]
+        lib.sco_block_elems.restype = C.c_int64
+        lib.sco_block_elems.argtypes = [C.c_int32] * 4
+        lib.sco_meu.argtypes = [C.c_int64, C.c_int64, i64p, i64p]
+        lib.sco_scale_up.restype = None
+        lib.sco_scale_up.argtypes = [C.c_int64] * 5 + [i64p, i64p]
+        lib.sco_scale_down.restype = None
+        lib.sco_scale_down.argtypes = [C.c_int64] * 5 + [i64p, i64p]
         _lib = lib
         return lib
 
@@ -95,6 +104,43 @@ def blocks_for(tokens: int, B: int) -> int:
 def append_count(hist_len: int, n_new: int, B: int) -> int:
     """O5: new table entries needed so the table covers hist_len+n_new tokens."""
     return int(_load().sco_append_count(hist_len, n_new, B))
+
+
+def lsc_rc_sizing(c_master: int, c_workers, m_block: int, L: int) -> dict:
+    """Eq. 2-5: LSC and RC capacities in blocks."""
+    cw = (C.c_int64 * max(len(c_workers), 1))(*c_workers)
+    out = (C.c_int64 * 6)()
+    if _load().sco_lsc_rc_sizing(c_master, cw, len(c_workers), m_block, L, out):
+        raise ValueError("sco_lsc_rc_sizing")
+    keys = ("k_master", "sum_k", "n_lsc", "n_rc", "max_context_blocks", "conventional_blocks")
+    return dict(zip(keys, (int(x) for x in out)))
+
+
+def block_elems(L: int, B: int, Hkv: int, D: int) -> int:
+    """Eq. 6 / 7 (PAPER.md:220-224)."""
+    return int(_load().sco_block_elems(L, B, Hkv, D))
+
+
+def meu(be_m: int, be_i: int):
+    """Eq. 8-9 (PAPER.md:298-304): (MEU_m, MEU_i)."""
+    a, b = C.c_int64(), C.c_int64()
+    if _load().sco_meu(be_m, be_i, C.byref(a), C.byref(b)):
+        raise ValueError("sco_meu")
+    return int(a.value), int(b.value)
+
+
+def scale_up(n_i, b_i, meu_i, meu_m, request_len):
+    """Algorithm 1 ScaleUp: (blocks the worker gains, blocks the master gives up)."""
+    a, b = C.c_int64(), C.c_int64()
+    _load().sco_scale_up(n_i, b_i, meu_i, meu_m, request_len, C.byref(a), C.byref(b))
+    return int(a.value), int(b.value)
+
+
+def scale_down(n_i, b_i, meu_i, meu_m, max_len):
+    """Algorithm 1 ScaleDown: (blocks the worker releases, blocks the master gains)."""
+    a, b = C.c_int64(), C.c_int64()
+    _load().sco_scale_down(n_i, b_i, meu_i, meu_m, max_len, C.byref(a), C.byref(b))
+    return int(a.value), int(b.value)
 
 
 class Pool:

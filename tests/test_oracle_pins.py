@@ -335,3 +335,74 @@ def test_multi_turn_tables_stay_disjoint_and_history_grows():
     for c in range(3):
         assert np.array_equal(pool.gather(0, 0, tables[c], hist[c]), logical[c][0])
         assert np.array_equal(pool.gather(0, 1, tables[c], hist[c]), logical[c][1])
+
+
+# ------------------------------------------------------------------ sizing and elasticity (O7)
+def test_lsc_rc_worked_example_from_the_paper():
+    """L=10, K_master=100, K_1=9, K_2=8 -> N_LSC=17, N_RC=8, 25 blocks vs 10."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "lsc_rc_worked_example.txt")) if l.strip() and l[0] != "#"]
+    for L, k_master, k1, k2, n_lsc, n_rc, total, conventional in (map(int, r) for r in rows):
+        m_block = 4096                                   # any block size gives the same counts
+        got = O.lsc_rc_sizing(k_master * m_block + 17, [k1 * m_block * L + 5, k2 * m_block * L], m_block, L)
+        assert (got["k_master"], got["sum_k"]) == (k_master, k1 + k2)
+        assert (got["n_lsc"], got["n_rc"], got["max_context_blocks"], got["conventional_blocks"]) == \
+               (n_lsc, n_rc, total, conventional)
+
+
+def test_lsc_fills_the_master_when_workers_offer_more():
+    """Eq. 4-5: sum K_i >= K_master -> N_LSC = K_master and no regular cache."""
+    got = O.lsc_rc_sizing(100 * 64, [90 * 64 * 4, 80 * 64 * 4], 64, 4)
+    assert (got["n_lsc"], got["n_rc"]) == (100, 0)
+    got = O.lsc_rc_sizing(100 * 64, [], 64, 4)           # no workers: all regular cache
+    assert (got["n_lsc"], got["n_rc"], got["conventional_blocks"]) == (0, 25, 25)
+
+
+def test_meu_is_the_lcm_split_brute_force():
+    """Eq. 8-9 against a brute-force search of the least common multiple."""
+    rng = np.random.default_rng(9)
+    for _ in range(200):
+        a, b = int(rng.integers(1, 400)), int(rng.integers(1, 400))
+        lcm = next(x for x in range(max(a, b), a * b + 1, max(a, b)) if x % a == 0 and x % b == 0)
+        mm, mi = O.meu(a, b)
+        assert mm * a == mi * b == lcm
+        assert math.gcd(mm, mi) == 1                     # the smallest such pair
+
+
+def test_meu_of_the_papers_models():
+    """Table 2 shapes: LWM 32/32/128 master, Qwen3-14B 40/8/128 worker, B=16."""
+    be_m, be_i = O.block_elems(32, 16, 32, 128), O.block_elems(40, 16, 8, 128)
+    assert (be_m, be_i) == (2097152, 655360)
+    assert O.meu(be_m, be_i) == (5, 16)                  # 5 master blocks == 16 worker blocks, in elements
+    assert O.meu(be_m, be_m) == (1, 1)
+
+
+@pytest.mark.parametrize("n_i,b_i,meu_i,meu_m,length,want", [
+    (10, 16, 3, 2, 160, (0, 0)),      # need 10 <= 10
+    (10, 16, 3, 2, 161, (3, 2)),      # need 11, diff 1, k 1
+    (10, 16, 3, 2, 200, (3, 2)),      # need 13, diff 3, k 1
+    (10, 16, 3, 2, 209, (6, 4)),      # need 14, diff 4, k 2
+    (0, 16, 16, 5, 1, (16, 5)),
+])
+def test_algorithm1_scale_up_hand_cases(n_i, b_i, meu_i, meu_m, length, want):
+    assert O.scale_up(n_i, b_i, meu_i, meu_m, length) == want
+
+
+@pytest.mark.parametrize("n_i,b_i,meu_i,meu_m,max_len,want", [
+    (20, 16, 3, 2, 320, (0, 0)),      # max_need 20 >= 20
+    (20, 16, 3, 2, 305, (0, 0)),      # max_need 20
+    (20, 16, 3, 2, 290, (0, 0)),      # max_need 19, diff 1, k 0
+    (20, 16, 3, 2, 100, (12, 8)),     # max_need 7, diff 13, k 4
+    (32, 16, 16, 5, 0, (32, 10)),
+])
+def test_algorithm1_scale_down_hand_cases(n_i, b_i, meu_i, meu_m, max_len, want):
+    assert O.scale_down(n_i, b_i, meu_i, meu_m, max_len) == want
+
+
+def test_scale_up_then_down_returns_whole_units():
+    """Both directions move multiples of (MEU_i, MEU_m) in the same ratio: no element is stranded."""
+    mm, mi = O.meu(O.block_elems(32, 16, 32, 128), O.block_elems(36, 16, 8, 128))
+    for length in (1, 500, 5000, 70000):
+        dw, dm = O.scale_up(7, 16, mi, mm, length)
+        assert dw % mi == 0 and dm % mm == 0 and dw // mi == dm // mm
+        bw, bm = O.scale_down(7 + dw, 16, mi, mm, 16 * 7)
+        assert bw % mi == 0 and bm % mm == 0 and bw // mi == bm // mm and bw <= dw
