@@ -238,6 +238,49 @@ sc_status_t sc_profile_collect(sc_pool_t *pool, double *ms_sum, int64_t *count);
 /* Number of kernels the library has launched since the pool was created (all kinds). */
 sc_status_t sc_launch_count(const sc_pool_t *pool, int64_t *n_launches);
 
+/* ------------------------------------------- sizing and elasticity (host integer logic)
+ * SURVEY.md 8(f) rows f3 and f1.  No device work, no data movement; all pointers HOST.   */
+
+typedef struct {
+    int64_t k_master;             /* Eq. 3: single-layer blocks the master's KV memory holds  */
+    int64_t sum_k;                /* sum of Eq. 2 over the workers: full-layer blocks offered */
+    int64_t n_lsc;                /* Eq. 4                                                    */
+    int64_t n_rc;                 /* Eq. 5                                                    */
+    int64_t max_context_blocks;   /* N_LSC + N_RC (x block_size = tokens)       */
+    int64_t conventional_blocks;  /* floor(K_master / L): a cache without the LSC             */
+} sc_sizing_t;
+
+/* PAPER.md:150-180 (Sec. 3.2, Eq. 1-5).  cfg gives the master's L, Hkv, D, B (M_block, Eq. 1);
+ * c_master_bytes / c_worker_bytes[i]: KV cache bytes of the master / the i-th worker.       */
+sc_status_t sc_lsc_rc_sizing(const sc_pool_config_t *cfg, int64_t c_master_bytes,
+                             const int64_t *c_worker_bytes, int32_t n_workers, sc_sizing_t *out);
+
+/* PAPER.md:218-304 (Sec. 3.4, Eq. 6-9): minimum elastic units.  Whenever the master moves
+ * *meu_master of its full-layer blocks, the worker moves *meu_worker of its own, and both are
+ * the same number of elements (their least common multiple).  Only n_layers, n_kv_heads,
+ * head_dim and block_size of the two configs are read.  SC_ERR_CAPACITY on int64 overflow.  */
+sc_status_t sc_elastic_units(const sc_pool_config_t *master, const sc_pool_config_t *worker,
+                             int64_t *meu_master, int64_t *meu_worker);
+
+/* PAPER.md:230-290 (Algorithm 1).  n_worker_blocks: blocks the worker holds now; block_size:
+ * the worker's; request_len / max_len: tokens of the incoming request / of the longest request
+ * of the last time window.  Outputs: blocks the worker gains (ScaleUp) or releases (ScaleDown)
+ * and the blocks the master gives up or gains, both multiples of the elastic units.          */
+sc_status_t sc_scale_up(int64_t n_worker_blocks, int32_t block_size, int64_t meu_worker,
+                        int64_t meu_master, int64_t request_len, int64_t *d_worker, int64_t *d_master);
+sc_status_t sc_scale_down(int64_t n_worker_blocks, int32_t block_size, int64_t meu_worker,
+                          int64_t meu_master, int64_t max_len, int64_t *d_worker, int64_t *d_master);
+
+/* PAPER.md:214-216 (block-major layout, Fig. 6): change the pool's capacity to new_n_blocks
+ * full-layer blocks WITHOUT moving any block.  Growing appends block ids n_blocks ..
+ * new_n_blocks-1 to the free list (the caller guarantees that the borrowed pool region
+ * now extends to new_pool_bytes >= new_n_blocks * block_bytes from the same pool_base; the new
+ * tail is zero-filled on `stream` if zero_fill != 0).  Shrinking releases the LAST blocks
+ * and is refused with SC_ERR_BAD_BLOCK_ID, changing nothing, unless every one of them is free
+ * (reading S17).  Offsets of surviving blocks (sc_cell_offset) do not change.               */
+sc_status_t sc_pool_resize(sc_pool_t *pool, int32_t new_n_blocks, size_t new_pool_bytes,
+                           int32_t zero_fill, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

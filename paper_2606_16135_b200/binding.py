@@ -38,7 +38,8 @@ SYMBOLS = [
     "sc_alloc_blocks", "sc_free_blocks", "sc_num_free_blocks", "sc_append_blocks", "sc_store_prefix",
     "sc_read_tokens", "sc_load_layer", "sc_prefill_layer", "sc_load_layer_batched",
     "sc_prefill_layer_batched", "sc_prefill_turn", "sc_launch_count", "sc_profile_enable",
-    "sc_profile_collect",
+    "sc_profile_collect", "sc_lsc_rc_sizing", "sc_elastic_units", "sc_scale_up", "sc_scale_down",
+    "sc_pool_resize",
 ]
 
 
@@ -53,6 +54,11 @@ class sc_pool_info_t(C.Structure):
     _fields_ = [("chunk_bytes", C.c_int64), ("cell_bytes", C.c_int64), ("block_bytes", C.c_int64),
                 ("pool_bytes", C.c_int64), ("lsc_buffer_bytes", C.c_int64), ("lsc_bytes", C.c_int64),
                 ("scratch_bytes", C.c_int64), ("n_free_blocks", C.c_int32), ("max_splits", C.c_int32)]
+
+
+class sc_sizing_t(C.Structure):
+    _fields_ = [("k_master", C.c_int64), ("sum_k", C.c_int64), ("n_lsc", C.c_int64), ("n_rc", C.c_int64),
+                ("max_context_blocks", C.c_int64), ("conventional_blocks", C.c_int64)]
 
 
 class SwiftCacheError(RuntimeError):
@@ -100,6 +106,11 @@ def lib() -> C.CDLL:
         "sc_launch_count": [vp, C.POINTER(i64)],
         "sc_profile_enable": [vp, i32],
         "sc_profile_collect": [vp, C.POINTER(C.c_double), C.POINTER(i64)],
+        "sc_lsc_rc_sizing": [C.POINTER(sc_pool_config_t), i64, C.POINTER(i64), i32, C.POINTER(sc_sizing_t)],
+        "sc_elastic_units": [C.POINTER(sc_pool_config_t), C.POINTER(sc_pool_config_t), C.POINTER(i64), C.POINTER(i64)],
+        "sc_scale_up": [i64, i32, i64, i64, i64, C.POINTER(i64), C.POINTER(i64)],
+        "sc_scale_down": [i64, i32, i64, i64, i64, C.POINTER(i64), C.POINTER(i64)],
+        "sc_pool_resize": [vp, i32, sz, i32, vp],
     }
     for name, argtypes in sig.items():
         fn = getattr(L, name)
@@ -127,6 +138,31 @@ def sc_pool_bytes_required(cfg: sc_pool_config_t):
     p, l = C.c_size_t(), C.c_size_t()
     check(lib().sc_pool_bytes_required(C.byref(cfg), C.byref(p), C.byref(l)))
     return int(p.value), int(l.value)
+
+
+def sc_lsc_rc_sizing(cfg: sc_pool_config_t, c_master_bytes: int, c_worker_bytes) -> dict:
+    cw = (C.c_int64 * max(len(c_worker_bytes), 1))(*c_worker_bytes)
+    out = sc_sizing_t()
+    check(lib().sc_lsc_rc_sizing(C.byref(cfg), c_master_bytes, cw, len(c_worker_bytes), C.byref(out)))
+    return {k: int(getattr(out, k)) for k, _ in sc_sizing_t._fields_}
+
+
+def sc_elastic_units(master: sc_pool_config_t, worker: sc_pool_config_t):
+    a, b = C.c_int64(), C.c_int64()
+    check(lib().sc_elastic_units(C.byref(master), C.byref(worker), C.byref(a), C.byref(b)))
+    return int(a.value), int(b.value)
+
+
+def sc_scale_up(n_worker_blocks, block_size, meu_worker, meu_master, request_len):
+    a, b = C.c_int64(), C.c_int64()
+    check(lib().sc_scale_up(n_worker_blocks, block_size, meu_worker, meu_master, request_len, C.byref(a), C.byref(b)))
+    return int(a.value), int(b.value)
+
+
+def sc_scale_down(n_worker_blocks, block_size, meu_worker, meu_master, max_len):
+    a, b = C.c_int64(), C.c_int64()
+    check(lib().sc_scale_down(n_worker_blocks, block_size, meu_worker, meu_master, max_len, C.byref(a), C.byref(b)))
+    return int(a.value), int(b.value)
 
 
 def make_config(L, Hq, Hkv, D, B, n_blocks, lsc_blocks, max_new_tokens, max_seqs=1,
@@ -181,6 +217,10 @@ class Pool:
 
     def set_split_tiles(self, tiles_per_split: int):
         check(lib().sc_set_split_tiles(self._h, tiles_per_split))
+
+    def resize(self, new_n_blocks: int, new_pool_bytes: int = 0, zero_fill: bool = True, stream=0):
+        check(lib().sc_pool_resize(self._h, new_n_blocks, new_pool_bytes, int(zero_fill), stream or None))
+        self.cfg.n_blocks = new_n_blocks
 
     def launch_count(self) -> int:
         n = C.c_int64()

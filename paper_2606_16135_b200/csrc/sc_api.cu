@@ -315,4 +315,134 @@ sc_status_t sc_append_blocks(sc_pool_t *pool, int32_t *table, int32_t *n_table, 
     return SC_OK;
 }
 
+// ---------------------------------------------- sizing and elasticity (f3, f1): host only
+namespace {
+
+// a * b for non-negative int64, false on overflow
+bool mul_ok(int64_t a, int64_t b, int64_t *r) { return !__builtin_mul_overflow(a, b, r); }
+
+sc_status_t block_elems_of(const sc_pool_config_t *c, int64_t *be)   // Eq. 6 / 7
+{
+    if (!c || c->n_layers <= 0 || c->block_size <= 0 || c->n_kv_heads <= 0 || c->head_dim <= 0)
+        return sc_fail(SC_ERR_INVALID_ARG, "config needs positive n_layers, block_size, n_kv_heads, head_dim");
+    int64_t v = c->n_layers;
+    if (!mul_ok(v, c->block_size, &v) || !mul_ok(v, c->n_kv_heads, &v) || !mul_ok(v, c->head_dim, &v))
+        return sc_fail(SC_ERR_CAPACITY, "block element count overflows int64");
+    *be = v;
+    return SC_OK;
+}
+
+}  // namespace
+
+sc_status_t sc_lsc_rc_sizing(const sc_pool_config_t *cfg, int64_t c_master_bytes,
+                             const int64_t *c_worker_bytes, int32_t n_workers, sc_sizing_t *out)
+{
+    if (!cfg || !out || n_workers < 0 || (n_workers > 0 && !c_worker_bytes) || c_master_bytes < 0)
+        return sc_fail(SC_ERR_INVALID_ARG, "bad argument");
+    if (cfg->n_layers <= 0 || cfg->block_size <= 0 || cfg->n_kv_heads <= 0 || cfg->head_dim <= 0)
+        return sc_fail(SC_ERR_INVALID_ARG, "config needs positive n_layers, block_size, n_kv_heads, head_dim");
+    // Eq. 1: one (block, layer) cell, K and V, bf16
+    const int64_t m_block = 2ll * cfg->block_size * cfg->n_kv_heads * cfg->head_dim * 2;
+    const int64_t full_layer_block = m_block * cfg->n_layers;
+    sc_sizing_t r;
+    r.k_master = c_master_bytes / m_block;                                   // Eq. 3
+    r.sum_k = 0;
+    for (int i = 0; i < n_workers; ++i) {
+        if (c_worker_bytes[i] < 0) return sc_fail(SC_ERR_INVALID_ARG, "worker %d: negative size", i);
+        r.sum_k += c_worker_bytes[i] / full_layer_block;                     // Eq. 2
+    }
+    const bool surplus = r.sum_k < r.k_master;
+    r.n_lsc = surplus ? r.sum_k : r.k_master;                                // Eq. 4
+    r.n_rc = surplus ? (r.k_master - r.sum_k) / cfg->n_layers : 0;           // Eq. 5
+    r.max_context_blocks = r.n_lsc + r.n_rc;
+    r.conventional_blocks = r.k_master / cfg->n_layers;
+    *out = r;
+    return SC_OK;
+}
+
+sc_status_t sc_elastic_units(const sc_pool_config_t *master, const sc_pool_config_t *worker,
+                             int64_t *meu_master, int64_t *meu_worker)
+{
+    if (!meu_master || !meu_worker) return sc_fail(SC_ERR_INVALID_ARG, "output pointer is NULL");
+    int64_t be_m, be_w;
+    sc_status_t st = block_elems_of(master, &be_m);
+    if (st) return st;
+    st = block_elems_of(worker, &be_w);
+    if (st) return st;
+    int64_t x = be_m, y = be_w;                       // Euclid
+    while (y != 0) { const int64_t t = x % y; x = y; y = t; }
+    // LCM/BE_m = BE_w/gcd and LCM/BE_w = BE_m/gcd (Eq. 8-9) -- no need to form the LCM itself
+    *meu_master = be_w / x;
+    *meu_worker = be_m / x;
+    return SC_OK;
+}
+
+sc_status_t sc_scale_up(int64_t n_worker_blocks, int32_t block_size, int64_t meu_worker,
+                        int64_t meu_master, int64_t request_len, int64_t *d_worker, int64_t *d_master)
+{
+    if (!d_worker || !d_master || n_worker_blocks < 0 || block_size <= 0 || meu_worker <= 0 || meu_master <= 0 ||
+        request_len < 0)
+        return sc_fail(SC_ERR_INVALID_ARG, "bad argument");
+    *d_worker = *d_master = 0;
+    const int64_t need = request_len / block_size + (request_len % block_size != 0);
+    if (need <= n_worker_blocks) return SC_OK;                                // enough capacity already
+    const int64_t missing = need - n_worker_blocks;
+    const int64_t units = missing / meu_worker + (missing % meu_worker != 0);  // whole elastic units, rounded up
+    if (!mul_ok(units, meu_worker, d_worker) || !mul_ok(units, meu_master, d_master))
+        return sc_fail(SC_ERR_CAPACITY, "block count overflows int64");
+    return SC_OK;
+}
+
+sc_status_t sc_scale_down(int64_t n_worker_blocks, int32_t block_size, int64_t meu_worker,
+                          int64_t meu_master, int64_t max_len, int64_t *d_worker, int64_t *d_master)
+{
+    if (!d_worker || !d_master || n_worker_blocks < 0 || block_size <= 0 || meu_worker <= 0 || meu_master <= 0 ||
+        max_len < 0)
+        return sc_fail(SC_ERR_INVALID_ARG, "bad argument");
+    *d_worker = *d_master = 0;
+    const int64_t max_need = max_len / block_size + (max_len % block_size != 0);
+    if (max_need >= n_worker_blocks) return SC_OK;                            // the allocation is still needed
+    const int64_t units = (n_worker_blocks - max_need) / meu_worker;          // whole elastic units, rounded down
+    if (!mul_ok(units, meu_worker, d_worker) || !mul_ok(units, meu_master, d_master))
+        return sc_fail(SC_ERR_CAPACITY, "block count overflows int64");
+    return SC_OK;
+}
+
+sc_status_t sc_pool_resize(sc_pool_t *pool, int32_t new_n_blocks, size_t new_pool_bytes,
+                           int32_t zero_fill, void *stream)
+{
+    if (!pool || new_n_blocks <= 0) return sc_fail(SC_ERR_INVALID_ARG, "bad argument");
+    std::lock_guard<std::mutex> lk(pool->mu);
+    const int32_t old_n = pool->cfg.n_blocks;
+    const size_t need = (size_t)new_n_blocks * (size_t)pool->g.block_bytes;
+    if (new_n_blocks == old_n) return SC_OK;
+    if (new_n_blocks > old_n) {
+        if (!pool->host_only && new_pool_bytes < need)
+            return sc_fail(SC_ERR_CAPACITY, "pool region %zu < %zu bytes", new_pool_bytes, need);
+        if (!pool->host_only && zero_fill) {
+            char *tail = pool->pool_base + (size_t)old_n * (size_t)pool->g.block_bytes;
+            const size_t bytes = need - (size_t)old_n * (size_t)pool->g.block_bytes;
+            if (pool->cfg.pool_kind == SC_POOL_HOST_PINNED) memset(tail, 0, bytes);
+            else SC_CUDA(cudaMemsetAsync(tail, 0, bytes, (cudaStream_t)stream));
+        }
+        // Block-major: the new blocks are simply the next ids.  They go to the FRONT
+        // of the free list (handed out last), so the tail stays free for a later shrink (S17).
+        std::vector<int32_t> fresh;
+        for (int32_t id = new_n_blocks - 1; id >= old_n; --id) fresh.push_back(id);
+        pool->free_list.insert(pool->free_list.begin(), fresh.begin(), fresh.end());
+        pool->allocated.resize(new_n_blocks, 0);
+    } else {
+        for (int32_t id = new_n_blocks; id < old_n; ++id)
+            if (pool->allocated[id])
+                return sc_fail(SC_ERR_BAD_BLOCK_ID, "cannot shrink to %d blocks: block %d is in use", new_n_blocks, id);
+        pool->free_list.erase(std::remove_if(pool->free_list.begin(), pool->free_list.end(),
+                                             [&](int32_t id) { return id >= new_n_blocks; }),
+                              pool->free_list.end());
+        pool->allocated.resize(new_n_blocks);
+    }
+    pool->cfg.n_blocks = new_n_blocks;
+    pool->pool_bytes = (int64_t)need;
+    return SC_OK;
+}
+
 }  // extern "C"

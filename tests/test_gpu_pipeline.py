@@ -225,3 +225,58 @@ def test_pipeline_ordering_survives_a_slow_stream(slow):
             assert_close(torch_to_bits(outs[turn][l]), refs[turn][l], f"slow {slow}: turn {turn} layer {l}")
     cv.check_pool_equals_logical()
     cv.sess.close()
+
+
+def test_block_major_resize_on_the_device():
+    """f1 (PAPER.md:214-216): growing the pool appends blocks and releasing the tail frees them;
+    no existing block moves -- the conversation's KV reads back bit-exactly through the same
+    table before and after, and the appended blocks are usable at once."""
+    L, Hkv, D, B = 3, 2, 128, 16
+    cfg = sc.make_config(L, 4, Hkv, D, B, 8, 0, 64)
+    pool_bytes8, _ = sc.sc_pool_bytes_required(cfg)
+    region = torch.full((pool_bytes8 // 8 * 12 + 1024,), 0x5A, dtype=torch.uint8, device="cuda")   # room for 12 blocks, dirty
+    off = (-region.data_ptr()) % 1024
+    base = region.data_ptr() + off
+    p = sc.Pool(cfg, base, pool_bytes8, 0, 0)
+    table = p.alloc_blocks(6)
+    tdev = torch.from_numpy(table.copy()).cuda()
+    T = 6 * B - 5
+    ks = [bits_to_torch(I.normal_bf16((T, Hkv, D), 300 + l), "cuda") for l in range(L)]
+    vs = [bits_to_torch(I.normal_bf16((T, Hkv, D), 400 + l), "cuda") for l in range(L)]
+    for l in range(L):
+        p.store_prefix(l, ks[l].data_ptr(), vs[l].data_ptr(), 0, T, tdev.data_ptr(), 6)
+
+    def read(l, tab, n_tab, start, n):
+        k = torch.empty((n, Hkv, D), dtype=torch.bfloat16, device="cuda")
+        v = torch.empty_like(k)
+        p.read_tokens(l, 0, tab.data_ptr(), n_tab, 0, start, n, k.data_ptr(), v.data_ptr())
+        torch.cuda.synchronize()
+        return k, v
+
+    p.resize(12, pool_bytes8 // 8 * 12)                        # grow: O(1), nothing moves
+    torch.cuda.synchronize()
+    for l in range(L):
+        k, v = read(l, tdev, 6, 0, T)
+        assert torch.equal(k.view(torch.int16), ks[l].view(torch.int16)) and torch.equal(v.view(torch.int16), vs[l].view(torch.int16))
+    raw = region[off:off + pool_bytes8 // 8 * 12]
+    assert int(raw[pool_bytes8:].max()) == 0                   # the appended tail was zero-filled
+    # the conversation grows into the appended blocks
+    more = p.alloc_blocks(4)
+    assert sorted(more.tolist()) == [6, 7, 8, 9]               # old free ids first, then the new ones
+    table2 = np.concatenate([table, more]).astype(np.int32)
+    t2 = torch.from_numpy(table2).cuda()
+    kn = bits_to_torch(I.normal_bf16((4 * B, Hkv, D), 500), "cuda")
+    vn = bits_to_torch(I.normal_bf16((4 * B, Hkv, D), 501), "cuda")
+    p.store_prefix(1, kn.data_ptr(), vn.data_ptr(), T, 4 * B, t2.data_ptr(), 10)
+    k, v = read(1, t2, 10, 0, T + 4 * B)
+    assert torch.equal(k.view(torch.int16), torch.cat([ks[1], kn]).view(torch.int16))
+    assert torch.equal(v.view(torch.int16), torch.cat([vs[1], vn]).view(torch.int16))
+    # release the tail: refused while block 9 is in use, fine once the tail is free
+    with pytest.raises(sc.SwiftCacheError):
+        p.resize(9)
+    p.free_blocks(more[more >= 8])
+    p.resize(8)                                                # blocks 6 and 7 stay allocated
+    for l in range(L):
+        k, v = read(l, tdev, 6, 0, T)
+        assert torch.equal(k.view(torch.int16), ks[l].view(torch.int16))
+    p.destroy()
