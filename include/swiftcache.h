@@ -255,6 +255,15 @@ typedef struct {
 sc_status_t sc_lsc_rc_sizing(const sc_pool_config_t *cfg, int64_t c_master_bytes,
                              const int64_t *c_worker_bytes, int32_t n_workers, sc_sizing_t *out);
 
+/* PAPER.md:174-178 (regular cache, RC): the first n_blocks logical blocks of every conversation
+ * are RESIDENT -- "stores KV cache directly on the master's local memory and retains full-layer
+ * data ... requires no cross-GPU transfer".  In STAGED mode sc_load_layer* then skips them
+ * (only later blocks are gathered into the LSC) and sc_prefill_layer* reads them in place
+ * through the block table; FUSED mode is unaffected.  Only complete history blocks count
+ * (min(n_blocks, hist_len / B) per conversation).  0 (default) = everything is streamed.
+ * tcgen05 engine only (SC_ERR_UNSUPPORTED from a staged call with the mma.sync engine).      */
+sc_status_t sc_set_resident_blocks(sc_pool_t *pool, int32_t n_blocks);
+
 /* PAPER.md:218-304 (Sec. 3.4, Eq. 6-9): minimum elastic units.  Whenever the master moves
  * *meu_master of its full-layer blocks, the worker moves *meu_worker of its own, and both are
  * the same number of elements (their least common multiple).  Only n_layers, n_kv_heads,

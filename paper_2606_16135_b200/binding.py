@@ -39,7 +39,7 @@ SYMBOLS = [
     "sc_read_tokens", "sc_load_layer", "sc_prefill_layer", "sc_load_layer_batched",
     "sc_prefill_layer_batched", "sc_prefill_turn", "sc_launch_count", "sc_profile_enable",
     "sc_profile_collect", "sc_lsc_rc_sizing", "sc_elastic_units", "sc_scale_up", "sc_scale_down",
-    "sc_pool_resize",
+    "sc_pool_resize", "sc_set_resident_blocks",
 ]
 
 
@@ -111,6 +111,7 @@ def lib() -> C.CDLL:
         "sc_scale_up": [i64, i32, i64, i64, i64, C.POINTER(i64), C.POINTER(i64)],
         "sc_scale_down": [i64, i32, i64, i64, i64, C.POINTER(i64), C.POINTER(i64)],
         "sc_pool_resize": [vp, i32, sz, i32, vp],
+        "sc_set_resident_blocks": [vp, i32],
     }
     for name, argtypes in sig.items():
         fn = getattr(L, name)
@@ -221,6 +222,9 @@ class Pool:
     def resize(self, new_n_blocks: int, new_pool_bytes: int = 0, zero_fill: bool = True, stream=0):
         check(lib().sc_pool_resize(self._h, new_n_blocks, new_pool_bytes, int(zero_fill), stream or None))
         self.cfg.n_blocks = new_n_blocks
+
+    def set_resident_blocks(self, n_blocks: int):
+        check(lib().sc_set_resident_blocks(self._h, n_blocks))
 
     def launch_count(self) -> int:
         n = C.c_int64()

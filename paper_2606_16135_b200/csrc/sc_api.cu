@@ -408,6 +408,13 @@ sc_status_t sc_scale_down(int64_t n_worker_blocks, int32_t block_size, int64_t m
     return SC_OK;
 }
 
+sc_status_t sc_set_resident_blocks(sc_pool_t *pool, int32_t n_blocks)
+{
+    if (!pool || n_blocks < 0) return sc_fail(SC_ERR_INVALID_ARG, "bad argument");
+    pool->resident_blocks = n_blocks;
+    return SC_OK;
+}
+
 sc_status_t sc_pool_resize(sc_pool_t *pool, int32_t new_n_blocks, size_t new_pool_bytes,
                            int32_t zero_fill, void *stream)
 {

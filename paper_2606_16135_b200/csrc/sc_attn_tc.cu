@@ -413,7 +413,10 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 #pragma unroll
                 for (int c = 0; c < 8; ++c) {
                     const int lb = min(j * 8 + c, nblk - 1);
-                    blk[c] = a.kv.base + sc_phys_block(a.kv, b, s, lb) * a.kv.block_stride;
+                    // a resident block (regular cache) is read in place, the rest from the LSC
+                    blk[c] = (a.has_res && lb < b.rc_blk[s])
+                                 ? a.kv_res.base + sc_phys_block(a.kv_res, b, s, lb) * a.kv_res.block_stride
+                                 : a.kv.base + sc_phys_block(a.kv, b, s, lb) * a.kv.block_stride;
                 }
 #pragma unroll
                 for (int kv = 0; kv < 2; ++kv) {

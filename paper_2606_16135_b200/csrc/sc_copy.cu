@@ -79,7 +79,7 @@ sc_gather_ldg_kernel(ScGeom g, ScBatch b, ScKvView src, ScKvView dst, int pieces
     const int gb = blockIdx.x / pieces_per_cell;
     const int piece = blockIdx.x - gb * pieces_per_cell;
     const int s = seq_of(b.cu_blk, b.n_seq, gb);
-    const int j = gb - b.cu_blk[s];
+    const int j = gb - b.cu_blk[s] + b.rc_blk[s];          // resident blocks are not gathered
     const char *sp = src.base + sc_phys_block(src, b, s, j) * src.block_stride;
     char *dp = dst.base + sc_phys_block(dst, b, s, j) * dst.block_stride;
     const int64_t off0 = (int64_t)piece * kGatherPiece + threadIdx.x * 16;
@@ -156,7 +156,7 @@ sc_gather_bulk_kernel(ScGeom g, ScBatch b, ScKvView src, ScKvView dst, int piece
         const int item = blockIdx.x + it * gridDim.x;
         const int gb = item / pieces_per_cell, piece = item - gb * pieces_per_cell;
         const int s = seq_of(b.cu_blk, b.n_seq, gb);
-        const int j = gb - b.cu_blk[s];
+        const int j = gb - b.cu_blk[s] + b.rc_blk[s];      // resident blocks are not gathered
         const int64_t off = (int64_t)piece * piece_bytes;
         sp = src.base + sc_phys_block(src, b, s, j) * src.block_stride + off;
         dp = dst.base + sc_phys_block(dst, b, s, j) * dst.block_stride + off;

@@ -44,6 +44,8 @@ struct ScBatch {
     int32_t lsc_off[SC_MAX_SEQS];     // first LSC block of each sequence
     int32_t cu_mt[SC_MAX_SEQS + 1];   // prefix sums of query M-tiles (engine specific)
     int32_t cu_blk[SC_MAX_SEQS + 1];  // prefix sums of blocks to copy (gather)
+    int32_t rc_blk[SC_MAX_SEQS];      // leading logical blocks that are RESIDENT (regular cache): never gathered,
+                                      // read in place through the table even in staged mode
     int32_t lsc_total;                // LSC blocks the whole batch occupies
 };
 
@@ -79,6 +81,7 @@ struct sc_pool {
 
     int32_t attn_engine = SC_ENGINE_AUTO, copy_engine = SC_COPY_AUTO;
     int32_t split_tiles_override = 0;
+    int32_t resident_blocks = 0;      // f3: leading blocks of every conversation kept as regular cache
     int32_t n_sms = 148;
 
     // pipeline resources (a8)
@@ -144,6 +147,8 @@ struct ScAttnArgs {
     const void *q;      // [sum n][Hq][D] bf16
     void *out;          // [sum n][Hq][D] bf16
     ScKvView kv;        // history + new tokens, through the table (or LSC identity)
+    ScKvView kv_res;    // staged mode with a regular cache: where logical blocks < rc_blk[s] are read (the pool)
+    int32_t has_res;
     float *part_o, *part_ml;
     // tcgen05 engine: the scatter of the new K/V (a5) is folded into the attention kernel
     const void *k_new, *v_new;   // [sum n][Hkv][D] bf16, or nullptr: already scattered

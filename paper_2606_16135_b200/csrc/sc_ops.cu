@@ -69,9 +69,10 @@ sc_status_t make_batch(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, 
         b->lsc_off[s] = lsc;
         b->cu_mt[s] = mt;
         b->cu_blk[s] = blk;
+        b->rc_blk[s] = std::min(p->resident_blocks, hist_lens[s] / p->g.B);   // complete history blocks only
         lsc += ceil_div((int)tot, p->g.B);
         mt += ceil_div(n, tile_m);
-        blk += ceil_div(hist_lens[s], p->g.B);
+        blk += ceil_div(hist_lens[s], p->g.B) - b->rc_blk[s];
     }
     b->cu_new[n_seq] = cu_new[n_seq];
     b->cu_mt[n_seq] = mt;
@@ -310,6 +311,9 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     a.part_ml = pool->part_ml;
     a.k_new = fold_scatter ? k_new : nullptr;
     a.v_new = fold_scatter ? v_new : nullptr;
+    a.kv_res = pv;
+    a.has_res = (staged && pool->resident_blocks > 0) ? 1 : 0;
+    if (a.has_res && !tc) return sc_fail(SC_ERR_UNSUPPORTED, "resident blocks in staged mode need the tcgen05 engine");
     a.scat0 = pv;
     a.scat1 = lv;
     a.has_scat1 = staged ? 1 : 0;

@@ -186,3 +186,36 @@ def test_argument_errors_launch_nothing():
         assert e.value.status == status, str(e.value)
     assert p.launch_count() == before
     c.close()
+
+
+# ------------------------------------------------------------------ f3: regular cache + LSC
+@pytest.mark.parametrize("resident", [1, 7, 10_000])
+def test_resident_leading_blocks_are_read_in_place(resident):
+    """the first N_RC blocks of a conversation stay resident; only the rest is
+    gathered into the LSC.  Same answer as streaming everything (bit for bit: same kernel, same
+    partitioning), and the LSC cells of the resident blocks are never written."""
+    T_h, n = 333, 70                                             # 20 complete history blocks + 13 tokens
+    base = Case(L=2, Hq=8, Hkv=2, D=128, T_h=T_h, n=n, NB=64, seed=88)
+    want = [base.run_layer(l, sc.SC_ATTN_STAGED, buf=l & 1) for l in range(2)]
+    refs = [base.oracle_layer(l) for l in range(2)]
+    base.close()
+    c = Case(L=2, Hq=8, Hkv=2, D=128, T_h=T_h, n=n, NB=64, seed=88)
+    c.sess.pool.set_resident_blocks(resident)
+    rc = min(resident, T_h // 16)
+    info = c.sess.pool.info()
+    for l in range(2):
+        got = c.run_layer(l, sc.SC_ATTN_STAGED, buf=l & 1)
+        assert np.array_equal(got, want[l])
+        assert_close(got, refs[l], f"resident {resident} layer {l}")
+        lsc = c.sess.lsc_mem.cpu().numpy()
+        buf0 = (l & 1) * info.lsc_buffer_bytes
+        assert not lsc[buf0:buf0 + rc * info.cell_bytes].any()                   # resident blocks: not gathered
+        assert lsc[buf0 + rc * info.cell_bytes:buf0 + (rc + 1) * info.cell_bytes].any()   # the next one was
+        k, v = c.sess.read_tokens(l, 0, c.table_dev, 0, T_h + n)                 # I2 still holds
+        assert np.array_equal(torch_to_bits(k), np.concatenate([c.data[l][1], c.data[l][3]]))
+        assert np.array_equal(torch_to_bits(v), np.concatenate([c.data[l][2], c.data[l][4]]))
+    with pytest.raises(sc.SwiftCacheError) as e:                                 # mma.sync engine: not supported
+        c.sess.pool.set_engine(sc.SC_ENGINE_MMA_SYNC, sc.SC_COPY_AUTO)
+        c.run_layer(0, sc.SC_ATTN_STAGED)
+    assert e.value.status == sc.SC_ERR_UNSUPPORTED
+    c.close()
