@@ -423,7 +423,7 @@ def run_ours(args):
     d_avg = avg(prof[dom])
     bound, amount = work[dom]
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.txt")
     if os.path.exists(tpath):
         with open(tpath) as f:
             traffic = json.load(f).get(f"{args.workload}:{dom}")
