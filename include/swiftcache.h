@@ -20,6 +20,9 @@
  *   - Data calls only ENQUEUE work on the given stream and return.  Ordering
  *     between different streams is the caller's job (or the pipeline
  *     helper's, sc_prefill_turn).
+ *   - Threads: the allocator / table calls of one pool are serialised internally; the data
+ *     calls of one pool (they share its scratch and counters) must come from one host
+ *     thread at a time.  Different pools are independent.
  *   - Ownership: the sc_pool_t object and its internal scratch belong to the
  *     library.  pool_base / lsc_base and every tensor or table pointer are
  *     BORROWED from the caller and never freed here (the pool is *donated*

@@ -49,6 +49,9 @@ constexpr float kRescaleThreshold = 8.f;   // log2 units
 // threads could have, so that a 128-thread gather CTA of the copy stream fits beside an
 // attention CTA on the same SM; warps 0-3 then shrink to 56 and the softmax warps grow to 200
 // (setmaxnreg).  LEAN = 0 (fused mode, nothing to share the SM with): 168 -> 72 / 208.
+// Either way 384 threads x >= 152 registers leave room for only ONE attention CTA per SM, also at
+// D = 64 where two would fit in shared memory: each CTA allocates all 512 TMEM columns, and two
+// CTAs of one cluster on the same SM would wait for each other (TMEM vs cluster barrier).
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
