@@ -78,8 +78,8 @@ sc_attn_mma_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     const int rows_valid = min(kTileM, n_s - i0);
     const int kmax = T_h + i0 + rows_valid;                 // keys [0, kmax) are visible to the tile
     const int tiles_needed = (kmax + kTileN - 1) / kTileN;
-    const int t_begin = split * a.split_tiles;
-    const int t_end = min(t_begin + a.split_tiles, tiles_needed);
+    const int t_begin = split * a.split_units;
+    const int t_end = min(t_begin + a.split_units, tiles_needed);
     if (t_begin >= t_end) return;
     const int nblk_s = (T_h + n_s + 15) >> 4;
     const int hk = h / (g.Hq / g.Hkv);
@@ -255,7 +255,7 @@ sc_attn_mma_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 // One warp per (row, head): O = sum_s 2^(m_s-M) O_s / sum_s 2^(m_s-M) l_s.
 template <int D>
 __global__ void __launch_bounds__(256)
-sc_combine_kernel(ScGeom g, ScBatch b, ScAttnArgs a, int tile_m, int tile_n)
+sc_combine_kernel(ScGeom g, ScBatch b, ScAttnArgs a, int tile_m, int split_unit)
 {
     const int64_t wid = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -268,8 +268,8 @@ sc_combine_kernel(ScGeom g, ScBatch b, ScAttnArgs a, int tile_m, int tile_n)
     const int mt = i / tile_m;
     const int rows_valid = min(tile_m, n_s - mt * tile_m);
     const int kmax = b.hist[s] + mt * tile_m + rows_valid;
-    const int tiles_needed = (kmax + tile_n - 1) / tile_n;
-    const int ns = (tiles_needed + a.split_tiles - 1) / a.split_tiles;
+    const int units_needed = (kmax + split_unit - 1) / split_unit;
+    const int ns = (units_needed + a.split_units - 1) / a.split_units;
     constexpr int V = D / 32;                                  // floats per lane
     float M = -INFINITY;
     for (int sp = 0; sp < ns; ++sp)
@@ -298,7 +298,7 @@ sc_combine_kernel(ScGeom g, ScBatch b, ScAttnArgs a, int tile_m, int tile_n)
 }  // namespace
 
 int sc_mma_tile_m() { return kTileM; }
-int sc_mma_tile_n() { return kTileN; }
+int sc_mma_split_unit() { return kTileN; }
 
 cudaError_t sc_launch_attn_mma(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st)
 {
@@ -322,12 +322,12 @@ cudaError_t sc_launch_attn_mma(const ScGeom &g, const ScBatch &b, const ScAttnAr
 }
 
 cudaError_t sc_launch_combine(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, int tile_m,
-                              int tile_n, cudaStream_t st)
+                              int split_unit, cudaStream_t st)
 {
     const int64_t warps = (int64_t)a.total_new * g.Hq;
     if (warps == 0) return cudaSuccess;
     const unsigned grid = (unsigned)((warps * 32 + 255) / 256);
-    if (g.D == 128) sc_combine_kernel<128><<<grid, 256, 0, st>>>(g, b, a, tile_m, tile_n);
-    else sc_combine_kernel<64><<<grid, 256, 0, st>>>(g, b, a, tile_m, tile_n);
+    if (g.D == 128) sc_combine_kernel<128><<<grid, 256, 0, st>>>(g, b, a, tile_m, split_unit);
+    else sc_combine_kernel<64><<<grid, 256, 0, st>>>(g, b, a, tile_m, split_unit);
     return cudaGetLastError();
 }

@@ -3,44 +3,50 @@
 // and including itself).
 //
 // One CTA owns a PAIR of 128-row query tiles of one query head (256 new tokens) and a
-// contiguous range of 128-token KV tiles (one split).  Warp roles:
-//   warp 0      producer : per KV tile, 8 + 8 bulk copies (cp.async.bulk, 4 KiB each) bring
-//                          the K and V chunks of the tile's 8 pool blocks -- found through the
-//                          block table -- into a 5-slot shared-memory ring.  The pool stores
-//                          chunks in the tensor core's 128B-swizzled operand order
+// contiguous range of 16-token pool blocks (one split), walked in KV tiles of 8 blocks; the
+// last tile of a split may hold fewer blocks (the MMAs then use N = 16 * blocks).  Warp roles:
+//   warp 0      producer : per KV tile, up to 8 + 8 bulk copies (cp.async.bulk, 4 KiB each)
+//                          bring the K and V chunks of the tile's pool blocks -- found through
+//                          the block table -- into a 5-slot shared-memory ring.  The pool
+//                          stores chunks in the tensor core's 128B-swizzled operand order
 //                          (include/swiftcache.h), so a chunk is an MMA operand as it lands.
 //   warp 1      MMA      : one thread issues tcgen05.mma.  S_m = Q_m K^T (both operands in
 //                          shared memory, K-major) into TMEM; O_m += P_m V with P_m read from
 //                          TMEM and V as an MN-major shared-memory operand.
 //   warp 2      TMEM allocation (all 512 columns: S0 S1 O0 O1, 128 fp32 columns each);
 //   warps 2-3   in cluster mode: this CTA's share of the scatter of the new K/V (a5)
-//   warps 4-7   softmax warpgroup of query tile 0: thread r owns row r.  tcgen05.ld S,
-//   warps 8-11  same for query tile 1            : mask, online softmax in registers with
-//                          lazy rescaling of O (only when the row max grows by > 2^8), P
-//                          rounded to bf16 and stored over S in TMEM, epilogue.
+//   warps 4-7   softmax warpgroup of query tile 0: thread r owns row r.  S is read from TMEM
+//   warps 8-11  same for query tile 1            : 32 columns at a time, online softmax in
+//                          registers against a LAZY reference maximum (advanced, and O
+//                          rescaled, only when the row max grows by > 2^8), P rounded to bf16
+//                          and stored over S in TMEM, epilogue.
 // The two query tiles ping-pong on the tensor pipe: while warpgroup 0 does the softmax of
 // tile j, the pipe runs PV and QK^T of query tile 1.
 //
 // Split-KV (a7): with up to 16 splits that fit one wave, the CTAs of one (query pair, head) are
 // a thread-block cluster; they share the scatter and merge their partial (m, l, O) through
-// distributed shared memory at the end.  Otherwise partials go to global scratch and
-// sc_combine_kernel merges them, and the scatter kernel runs before this one.
+// distributed shared memory at the end (row-scaled fp16 partials moved by the TMA engine).
+// Otherwise partials go to global scratch and sc_combine_kernel merges them, and the scatter
+// kernel runs before this one.
 //
 // Work partitioning depends on logical positions only, so results are bit-identical under
 // any permutation of physical block ids, and staged attention is this same kernel run with
 // the identity table over the LSC.
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <stdlib.h>
 
 #include <type_traits>
 
 #include "sc_internal.h"
+#include "sc_probe.h"
 
 namespace {
 
 constexpr int kTM = 128;          // rows of one query tile
 constexpr int kPairM = 2 * kTM;   // rows a CTA owns
-constexpr int kTN = 128;          // KV tokens per tile (8 pool blocks)
+constexpr int kTN = 128;          // KV tokens per full tile (8 pool blocks)
+constexpr int kTileBlks = 8;
 constexpr int kStages = 5;        // ring slots (each holds the K or the V half of a tile)
 constexpr int kThreads = 384;
 constexpr int kMaxCluster = 16;   // most splits merged in kernel (non-portable cluster size)
@@ -72,7 +78,11 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
 }
 // A wait that cannot hang the GPU: after ~2 s of failed probes the kernel traps (surfaces as
-// SC_ERR_CUDA on the next call) instead of spinning forever on a protocol error.
+// SC_ERR_CUDA on the next call) instead of spinning forever on a protocol error.  Each probe
+// carries a suspend-time hint: the thread sleeps in hardware until the phase completes (or the
+// hint runs out) instead of polling -- a polling warp takes issue slots from the softmax warp
+// that shares its scheduler.
+constexpr uint32_t kSuspendNs = 200000;
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;
@@ -80,16 +90,16 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
     for (;;) {
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
             "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+            : "=r"(ok) : "r"(bar), "r"(parity), "r"(kSuspendNs) : "memory");
         if (ok) return;
         const long long t = clock64();
         if (t0 == 0) t0 = t;
         else if (t - t0 > 4000000000ll) __trap();
     }
 }
-// same, acquiring at cluster scope (the arrivals come from other CTAs of the cluster)
+// same, acquiring at cluster scope (the arrivals / bytes come from other CTAs of the cluster)
 __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;
@@ -97,9 +107,9 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
     for (;;) {
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2, %3;\n\t"
             "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+            : "=r"(ok) : "r"(bar), "r"(parity), "r"(kSuspendNs) : "memory");
         if (ok) return;
         const long long t = clock64();
         if (t0 == 0) t0 = t;
@@ -112,13 +122,25 @@ __device__ __forceinline__ void bulk_g2s(uint32_t smem_dst, const void *gsrc, ui
         "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
         :: "r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar) : "memory");
 }
+// this CTA's shared memory -> a peer CTA's shared memory (destination and barrier are addresses
+// in the shared::cluster window of the peer), completing on the PEER's mbarrier
+__device__ __forceinline__ void bulk_s2peer(uint32_t peer_dst, uint32_t src, uint32_t bytes, uint32_t peer_bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        :: "r"(peer_dst), "r"(src), "r"(bytes), "r"(peer_bar) : "memory");
+}
+__device__ __forceinline__ uint32_t mapa(uint32_t addr, int cta)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(cta));
+    return r;
+}
 
 // all threads of all CTAs of the cluster; release / acquire at cluster scope (global writes included)
-__device__ __forceinline__ void cluster_sync_all()
-{
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_sync_all() { cluster_arrive(); cluster_wait(); }
 
 // ------------------------------------------------------------------ tcgen05
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -184,6 +206,36 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
            "r"(taddr) : "memory");
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// tcgen05.wait::ld naming the registers the load is still writing as in/out operands: nothing
+// that reads them can be scheduled above the wait.
+__device__ __forceinline__ void tmem_ld_wait(uint32_t (&r)[32])
+{
+    asm volatile(
+        "tcgen05.wait::ld.sync.aligned;"
+        : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+          "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15]),
+          "+r"(r[16]), "+r"(r[17]), "+r"(r[18]), "+r"(r[19]), "+r"(r[20]), "+r"(r[21]), "+r"(r[22]), "+r"(r[23]),
+          "+r"(r[24]), "+r"(r[25]), "+r"(r[26]), "+r"(r[27]), "+r"(r[28]), "+r"(r[29]), "+r"(r[30]), "+r"(r[31])
+        :: "memory");
+}
+// 32 lanes x 16 columns (the pipelined softmax reads S in pieces of 16 columns)
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait(uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.wait::ld.sync.aligned;"
+        : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+          "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
+        :: "memory");
+}
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // ---- packed fp32x2 arithmetic (FFMA2 / FADD2 on sm_100): halves the FMA-pipe instructions of the softmax ----
@@ -209,10 +261,25 @@ __device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b)
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
     return d;
 }
+__device__ __forceinline__ float max3(float a, float b, float c)      // FMNMX3 on sm_100
+{
+    float d;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
 {
     __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
     return *reinterpret_cast<uint32_t *>(&v);
+}
+__device__ __forceinline__ uint32_t pack_f16(float lo, float hi)
+{
+    __half2 v = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<uint32_t *>(&v);
+}
+__device__ __forceinline__ float2 unpack_f16(uint32_t u)
+{
+    return __half22float2(*reinterpret_cast<__half2 *>(&u));
 }
 __device__ __forceinline__ int seq_of(const int32_t *cu, int n_seq, int x)
 {
@@ -222,16 +289,29 @@ __device__ __forceinline__ int seq_of(const int32_t *cu, int n_seq, int x)
 }
 
 // shared-memory plan (offsets from the 1024-byte aligned base)
+//   [kQOff]     Q_0, Q_1 (swizzled like K tiles); in the cluster epilogue: this CTA's partial O, one
+//               row-scaled fp16 row of D values per query row, 16-byte units XORed with the row index
+//   [kRingOff]  the KV ring; in the cluster epilogue: what the peers send, [split][row][D] fp16 and,
+//               from kRecvMlOff, [split][row] (A, L)
+//   [kBarOff]   mbarriers, TMEM base
+//   [kMlOff]    this CTA's (A, L) per query row (cluster epilogue)
 template <int D>
 struct Plan {
     static constexpr int NH = D / 64;
     static constexpr int kChunk = 16 * D * 2;          // one (block, head) chunk
     static constexpr int kQTile = kTM * D * 2;         // one query tile, swizzled like a K tile
     static constexpr int kSlot = kTN * D * 2;          // K (or V) of one KV tile = 8 chunks
+    static constexpr int kRowB = D * 2;                // one fp16 row of a partial O
+    static constexpr int kRecvRows = kPairM + 2 * kMaxCluster;   // rows_per_cta (even) * splits <= this
     static constexpr int kQOff = 0;
     static constexpr int kRingOff = 2 * kQTile;
+    static constexpr int kRecvMlOff = kRecvRows * kRowB;          // inside the ring
     static constexpr int kBarOff = kRingOff + kStages * kSlot;
-    static constexpr int kBytes = kBarOff + 256 + 1024;   // + barriers + alignment slack
+    static constexpr int kMlOff = kBarOff + 192;
+    static constexpr int kSlack = 832;                 // the dynamic window may start this far off a 1 KiB boundary
+    static constexpr int kBytes = kMlOff + kPairM * 8 + kSlack;
+    static_assert(kRecvMlOff + kRecvRows * 8 <= kStages * kSlot, "receive area must fit in the ring");
+    static_assert(kBytes <= 232448, "more than 227 KB of shared memory");
 };
 
 struct Bars {                       // at Plan::kBarOff
@@ -240,23 +320,10 @@ struct Bars {                       // at Plan::kBarOff
     uint64_t p_ready[2];            // softmax warpgroup m -> MMA: P_m stored, O_m rescaled
     uint64_t q_ready[2];            // Q_m in shared memory
     uint64_t scat_done;             // warps 2-3 -> producer: this CTA's share of the new K/V is in the pool
+    uint64_t recv;                  // cluster epilogue: the peers' partials have landed in this CTA
     uint32_t tmem_base;
 };
-
-#ifdef SC_TC_PROBE
-__constant__ int sc_probe_flags;
-__device__ long long sc_tl[256][64];
-#define PROBE(bit) (sc_probe_flags & (1 << (bit)))
-#define TL(i) do { const int cta_ = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z); \
-                   if (cta_ < 256) sc_tl[cta_][(i)] = clock64(); } while (0)
-#define TLG(i) do { const int cta_ = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z); \
-                    long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); \
-                    if (cta_ < 256) sc_tl[cta_][(i)] = t_; } while (0)
-#else
-#define PROBE(bit) 0
-#define TL(i) do { } while (0)
-#define TLG(i) do { } while (0)
-#endif
+static_assert(sizeof(Bars) <= 192, "Bars outgrew its slot");
 
 template <int D, int LEAN>
 __global__ void __maxnreg__(LEAN ? 152 : 168)
@@ -267,6 +334,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     extern __shared__ char smem_raw[];
     const uint32_t raw_u32 = smem_u32(smem_raw);
     const uint32_t base = (raw_u32 + 1023u) & ~1023u;
+    if (base - raw_u32 > (uint32_t)P::kSlack) __trap();          // never seen: the window starts on a 1 KiB boundary
     char *smem = smem_raw + (base - raw_u32);
     Bars *bars = reinterpret_cast<Bars *>(smem + P::kBarOff);
 
@@ -277,28 +345,30 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     const int n_s = b.cu_new[s + 1] - b.cu_new[s];
     const int T_h = b.hist[s];
     const int tok0 = pair * kPairM;
-    int rows[2], need[2], nt[2];
+    int rows[2], need[2], nt[2];                 // need: pool blocks query tile m can see
 #pragma unroll
     for (int m = 0; m < 2; ++m) {
         rows[m] = max(0, min(kTM, n_s - tok0 - m * kTM));
-        need[m] = rows[m] > 0 ? (T_h + tok0 + m * kTM + rows[m] + kTN - 1) / kTN : 0;
+        need[m] = rows[m] > 0 ? (T_h + tok0 + m * kTM + rows[m] + 15) >> 4 : 0;
     }
     const int need_max = max(need[0], need[1]);
-    const int t_begin = split * a.split_tiles;
-    if (t_begin >= need_max) {                   // no keys for this split: only keep the cluster barriers whole
+    const int b_begin = split * a.split_units;   // this split's blocks are [b_begin, b_end)
+    if (b_begin >= need_max) {                   // no keys for this split: only keep the cluster barriers whole
         if (a.cluster_combine) { cluster_sync_all(); cluster_sync_all(); cluster_sync_all(); }
         return;
     }
-    const int t_end = min(t_begin + a.split_tiles, need_max);
-    const int nt_max = t_end - t_begin;
+    const int b_end = min(b_begin + a.split_units, need_max);
+    const int nt_max = (b_end - b_begin + kTileBlks - 1) / kTileBlks;
 #pragma unroll
-    for (int m = 0; m < 2; ++m) nt[m] = max(0, min(t_end, need[m]) - t_begin);
+    for (int m = 0; m < 2; ++m) nt[m] = max(0, (min(b_end, need[m]) - b_begin + kTileBlks - 1) / kTileBlks);
+    const int ns_act = (need_max + a.split_units - 1) / a.split_units;        // CTAs of the pair that hold keys
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) { TL(0); TLG(60); }
     const uint32_t bar_full = smem_u32(&bars->full[0]), bar_empty = smem_u32(&bars->empty[0]);
     const uint32_t bar_s = smem_u32(&bars->s_ready[0]), bar_p = smem_u32(&bars->p_ready[0]);
     const uint32_t bar_q = smem_u32(&bars->q_ready[0]), bar_scat = smem_u32(&bars->scat_done);
+    const uint32_t bar_recv = smem_u32(&bars->recv);
     const uint32_t q_smem = base + P::kQOff, ring = base + P::kRingOff;
 
     if (threadIdx.x == 0) {
@@ -308,7 +378,8 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             mbar_init(bar_p + 8 * m, kTM);
             mbar_init(bar_q + 8 * m, kTM);
         }
-        mbar_init(bar_scat, a.cluster_combine ? 64 * ((need_max + a.split_tiles - 1) / a.split_tiles) : 256);
+        mbar_init(bar_scat, a.cluster_combine ? 64 * ns_act : 256);
+        mbar_init(bar_recv, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
@@ -321,32 +392,37 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     else __syncthreads();
     tc_fence_after();
     const uint32_t tmem = bars->tmem_base;
+    // Programmatic dependent launch: everything above overlapped the tail of the kernel before this
+    // one in the stream; nothing below may start until that kernel's memory is visible (q, k_new,
+    // v_new of this layer come from it in a model).  Then let the NEXT kernel begin its own set-up.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (threadIdx.x == 128) TL(1);
     float fin_m = -INFINITY, fin_l = 0.f;      // softmax threads: final (m in log2 units, l) of their row
 
     // ---- scatter (a5) ----
-    // Without a cluster: the softmax warps do it first; the CTA stores the new tokens at positions [p_lo, p_hi) -- those inside
-    // its own KV tiles that its query tiles can see -- and only relies on its own stores.
-    // With a cluster (one CTA per split of this query pair and head): the pair's new tokens are
-    // dealt out evenly over the cluster's CTAs, whose otherwise idle warps 2-3 store them in the
-    // background, and each thread then arrives (release, cluster
-    // scope) on the scat_done barrier of every CTA of the cluster; a producer waits for all of
-    // them before it loads the first KV tile that holds new tokens.  CTAs of other query heads
-    // of the group or of later query pairs may store the same bytes to the same places.
-    const int ns_act = (need_max + a.split_tiles - 1) / a.split_tiles;        // CTAs of the pair that hold keys
+    // The pair's new tokens [T_h, T_h + ntok) are stored into the pool (and the LSC tail in staged
+    // mode); the CTA of a sequence's LAST pair also zero-fills the rest of the last block, so that
+    // slots past the logical end hold finite values whatever the memory held before (they are
+    // masked in S, but 0 * NaN in P.V would poison the row).
+    // Without a cluster (one CTA per pair): the softmax warps do it first, overlapped with the Q loads.
+    // With a cluster (one CTA per split of this query pair and head): the rows are dealt out evenly
+    // over the cluster's CTAs, whose otherwise idle warps 2-3 store them in the background, and each
+    // thread then arrives (release, cluster scope) on the scat_done barrier of every CTA of the
+    // cluster; a producer waits for all of them before it loads the first KV tile that holds new
+    // tokens.  CTAs of other query heads of the group or of later query pairs may store the same
+    // bytes to the same places.
     auto scatter_share = [&](auto nthreads_c, int tid, auto &&after_first_loads) {
         constexpr int NT = decltype(nthreads_c)::value;
         if (a.k_new == nullptr) { after_first_loads(); return; }
         bool mid_done = false;
-        const int ntok_pair = min(n_s, tok0 + kPairM);
-        int p_lo, ntok, rest_lo, rest_hi;                            // rows of [K rows ; V rows] to store
+        const int ntok = min(n_s, tok0 + kPairM);                    // new tokens up to the end of this pair
+        const int npad = (tok0 + kPairM >= n_s) ? ((-(T_h + n_s)) & 15) : 0;
+        const int nall = ntok + npad;                                // rows of [K rows ; V rows] are 2 * nall
+        int rest_lo = 0, rest_hi = 2 * nall;
         if (a.cluster_combine) {
-            p_lo = T_h; ntok = ntok_pair;
-            const int per = (2 * ntok + ns_act - 1) / ns_act;
-            rest_lo = split * per; rest_hi = min(2 * ntok, rest_lo + per);
-        } else {
-            p_lo = max(T_h, kTN * t_begin); ntok = min(T_h + ntok_pair, kTN * t_end) - p_lo;
-            rest_lo = 0; rest_hi = 2 * ntok;
+            const int per = (2 * nall + ns_act - 1) / ns_act;
+            rest_lo = split * per; rest_hi = min(2 * nall, rest_lo + per);
         }
         if (rest_lo < rest_hi) {
             constexpr int CPR = D / 8;                              // 16-byte units per head row
@@ -359,11 +435,14 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 #pragma unroll
                 for (int k = 0; k < U; ++k) {
                     const int rest = r0 + k * RPI;
+                    val[k] = make_int4(0, 0, 0, 0);
                     if (rest < rest_hi) {
-                        const int kv = rest >= ntok, t = rest - kv * ntok;
-                        const int64_t row = (int64_t)b.cu_new[s] + (p_lo + t - T_h);
-                        val[k] = __ldg(reinterpret_cast<const int4 *>(
-                            (const char *)(kv ? a.v_new : a.k_new) + ((row * g.Hkv + hk) * D + c * 8) * 2));
+                        const int kv = rest >= nall, t = rest - kv * nall;
+                        if (t < ntok) {
+                            const int64_t row = (int64_t)b.cu_new[s] + t;
+                            val[k] = __ldg(reinterpret_cast<const int4 *>(
+                                (const char *)(kv ? a.v_new : a.k_new) + ((row * g.Hkv + hk) * D + c * 8) * 2));
+                        }
                     }
                 }
                 if (!mid_done) { after_first_loads(); mid_done = true; }   // overlaps this round trip
@@ -371,8 +450,8 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 for (int k = 0; k < U; ++k) {
                     const int rest = r0 + k * RPI;
                     if (rest < rest_hi) {
-                        const int kv = rest >= ntok, t = rest - kv * ntok;
-                        const int tok = p_lo + t, lb = tok >> 4, slot = tok & 15;
+                        const int kv = rest >= nall, t = rest - kv * nall;
+                        const int tok = T_h + t, lb = tok >> 4, slot = tok & 15;
                         const int64_t in_cell = (int64_t)(kv * g.Hkv + hk) * P::kChunk + sc_chunk_off(slot, c * 8, NH);
                         *reinterpret_cast<int4 *>(a.scat0.base + sc_phys_block(a.scat0, b, s, lb) * a.scat0.block_stride + in_cell) = val[k];
                         if (a.has_scat1)
@@ -384,11 +463,8 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         }
         if (!mid_done) after_first_loads();
         if (a.cluster_combine) {
-            for (int dst = 0; dst < ns_act; ++dst) {
-                uint32_t rbar;
-                asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbar) : "r"(bar_scat), "r"(dst));
-                asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(rbar) : "memory");
-            }
+            for (int dst = 0; dst < ns_act; ++dst)
+                asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(mapa(bar_scat, dst)) : "memory");
         } else {
             mbar_arrive(bar_scat);
         }
@@ -401,21 +477,21 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     if (warp == 0) {
         // =============================== producer ===============================
         if (lane == 0) {
-            const int nblk = (T_h + n_s + 15) >> 4;
             const int hk = h / (g.Hq / g.Hkv);
             const int64_t off_kv[2] = {(int64_t)hk * P::kChunk, (int64_t)(g.Hkv + hk) * P::kChunk};
             bool scat_waited = (a.k_new == nullptr);
             for (int jj = 0; jj < nt_max; ++jj) {
-                const int j = t_begin + jj;
-                if (!scat_waited && j >= T_h / kTN) {      // first tile with a block the scatter touches
+                const int tb = b_begin + jj * kTileBlks;         // first block of the tile
+                const int nbt = min(kTileBlks, b_end - tb);      // blocks it holds
+                if (!scat_waited && tb + nbt > (T_h >> 4)) {     // first tile with a block the scatter touches
                     mbar_wait_cluster(bar_scat, 0);
                     asm volatile("fence.proxy.async.global;" ::: "memory");   // generic-proxy stores -> bulk-copy reads
                     scat_waited = true;
                 }
-                const char *blk[8];
+                const char *blk[kTileBlks];
 #pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    const int lb = min(j * 8 + c, nblk - 1);
+                for (int c = 0; c < kTileBlks; ++c) {
+                    const int lb = min(tb + c, b_end - 1);
                     // a resident block (regular cache) is read in place, the rest from the LSC
                     blk[c] = (a.has_res && lb < b.rc_blk[s])
                                  ? a.kv_res.base + sc_phys_block(a.kv_res, b, s, lb) * a.kv_res.block_stride
@@ -426,11 +502,12 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     const int it = 2 * jj + kv, slot = it % kStages;
                     mbar_wait(bar_empty + 8 * slot, ((it / kStages) & 1) ^ 1);
                     if (PROBE(4)) { mbar_arrive(bar_full + 8 * slot); continue; }
-                    mbar_expect_tx(bar_full + 8 * slot, P::kSlot);
+                    mbar_expect_tx(bar_full + 8 * slot, (uint32_t)nbt * P::kChunk);
 #pragma unroll
-                    for (int c = 0; c < 8; ++c)
-                        bulk_g2s(ring + slot * P::kSlot + c * P::kChunk, blk[c] + off_kv[kv], P::kChunk,
-                                 bar_full + 8 * slot);
+                    for (int c = 0; c < kTileBlks; ++c)
+                        if (c < nbt)
+                            bulk_g2s(ring + slot * P::kSlot + c * P::kChunk, blk[c] + off_kv[kv], P::kChunk,
+                                     bar_full + 8 * slot);
                     if (it == 0) {
                         // The first MMA needs Q and K of tile 0 only.  All CTAs start together, so
                         // the rest of the ring is requested once Q has landed: it would only queue
@@ -446,9 +523,9 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     } else if (warp == 1) {
         // =============================== MMA issuer ===============================
         if (lane == 0) {
-            constexpr uint32_t idesc_qk = make_idesc(kTN, 0), idesc_pv = make_idesc(D, 1);
-            auto issue_qk = [&](int m, uint32_t kslot) {
+            auto issue_qk = [&](int m, uint32_t kslot, int nbt) {
                 if (PROBE(3)) return;
+                const uint32_t idesc_qk = make_idesc(16 * nbt, 0);
 #pragma unroll
                 for (int hf = 0; hf < NH; ++hf)
 #pragma unroll
@@ -458,25 +535,28 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                                 make_desc(kslot + o, 16, NH * 1024), idesc_qk, (hf | kk) != 0);
                     }
             };
-            auto issue_pv = [&](int m, uint32_t vslot, bool acc) {
+            auto issue_pv = [&](int m, uint32_t vslot, bool acc, int nbt) {
                 if (PROBE(2)) return;
+                constexpr uint32_t idesc_pv = make_idesc(D, 1);
 #pragma unroll
-                for (int kk = 0; kk < 8; ++kk)
-                    umma_ts(tmem + 256 + m * 128, tmem + m * 128 + kk * 8,
-                            make_desc(vslot + kk * P::kChunk, 1024, NH * 1024), idesc_pv, acc || kk != 0);
+                for (int kk = 0; kk < kTileBlks; ++kk)             // one MMA consumes one pool block
+                    if (kk < nbt)
+                        umma_ts(tmem + 256 + m * 128, tmem + m * 128 + kk * 8,
+                                make_desc(vslot + kk * P::kChunk, 1024, NH * 1024), idesc_pv, acc || kk != 0);
             };
             auto slot_addr = [&](int it) { return ring + (it % kStages) * P::kSlot; };
             auto wait_full = [&](int it) {
                 mbar_wait(bar_full + 8 * (it % kStages), (it / kStages) & 1);
                 tc_fence_after();
             };
+            auto blocks_of = [&](int jj) { return min(kTileBlks, b_end - (b_begin + jj * kTileBlks)); };
             // prologue: S_m = Q_m K_0^T
             wait_full(0);
 #pragma unroll
             for (int m = 0; m < 2; ++m)
                 if (nt[m] > 0) {
                     mbar_wait(bar_q + 8 * m, 0);
-                    issue_qk(m, slot_addr(0));
+                    issue_qk(m, slot_addr(0), blocks_of(0));
                     umma_commit(bar_s + 8 * m);
                 }
             umma_commit(bar_empty + 8 * (0 % kStages));
@@ -489,10 +569,10 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     if (jj >= nt[m]) continue;
                     mbar_wait(bar_p + 8 * m, jj & 1);
                     tc_fence_after();
-                    issue_pv(m, slot_addr(itv), jj > 0);
+                    issue_pv(m, slot_addr(itv), jj > 0, blocks_of(jj));
                     if (jj + 1 < nt[m]) {
                         if (!k_waited) { wait_full(itk); k_waited = true; }
-                        issue_qk(m, slot_addr(itk));
+                        issue_qk(m, slot_addr(itk), blocks_of(jj + 1));
                     }
                     umma_commit(bar_s + 8 * m);      // S_m(jj+1) ready, or: O_m final
                 }
@@ -557,42 +637,42 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         const uint32_t s_addr = tmem + lane_base + m * 128, o_addr = tmem + lane_base + 256 + m * 128;
         float m_used = -INFINITY, l_run = 0.f;
         for (int jj = 0; jj < nt[m]; ++jj) {
-            const int j = t_begin + jj;
+            const int tb = b_begin + jj * kTileBlks;
+            const int ncols = 16 * min(kTileBlks, b_end - tb);   // keys in this tile
             mbar_wait(bar_s + 8 * m, jj & 1);
             tc_fence_after();
             if (threadIdx.x == 128 && jj < 12) TL(3 + 2 * jj);
             if (threadIdx.x == 256 && jj < 12) TL(40 + jj);
             if (PROBE(1)) { tc_fence_before(); mbar_arrive(bar_p + 8 * m); continue; }
+            // last visible column of this row inside the tile; columns past the tile's keys hold
+            // stale values, so a tile with fewer than 128 keys is treated as masked
+            const int limit = min(T_h + row0 + r - 16 * tb, ncols - 1);
+            const bool masked_tile = (16 * tb + ncols - 1 > T_h + row0) || ncols < kTN;
+            // S of this row: all columns at once (one tcgen05.wait::ld per tile), masked where the tile
+            // crosses the causal boundary or holds fewer than 128 keys.
             uint32_t sv[kTN];
 #pragma unroll
             for (int c4 = 0; c4 < kTN / 32; ++c4)
                 tmem_ld32(s_addr + c4 * 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[c4 * 32]));
             tmem_ld_wait();
-            if (j * kTN + kTN - 1 > T_h + row0) {               // tile reaches past the first row's limit
-                const int limit = T_h + row0 + r - j * kTN;     // last visible column of this row
+            if (masked_tile) {
 #pragma unroll
                 for (int c = 0; c < kTN; ++c)
-                    if (c > limit) sv[c] = 0xff800000u;         // -inf
-            }
-            if (PROBE(0)) {
-                tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&sv[0]));
-                tmem_st32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[32]));
-                tmem_st_wait();
-                tc_fence_before();
-                mbar_arrive(bar_p + 8 * m);
-                continue;
+                    if (c > limit) sv[c] = 0xff800000u;             // -inf
             }
             float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};     // 4 chains: ILP
 #pragma unroll
             for (int c = 0; c < kTN; c += 8)
 #pragma unroll
                 for (int k = 0; k < 4; ++k)
-                    mx4[k] = fmaxf(mx4[k], fmaxf(__uint_as_float(sv[c + 2 * k]), __uint_as_float(sv[c + 2 * k + 1])));
+                    mx4[k] = max3(mx4[k], __uint_as_float(sv[c + 2 * k]), __uint_as_float(sv[c + 2 * k + 1]));
             const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
             const float m_new = fmaxf(m_used, mx);
+            // P = 2^(s*sl - m_used*sl).  The reference m_used is LAZY: it is only advanced (and O
+            // rescaled) when the row max has grown by more than 2^8, so P <= 256.
             const bool grow_max = (m_new - m_used) * sl > kRescaleThreshold;   // false for -inf - -inf (NaN)
             if (jj == 0) {
-                m_used = m_new;                                 // O_m not accumulated yet
+                m_used = m_new;                                     // O_m not accumulated yet
             } else if (__any_sync(0xffffffffu, grow_max)) {
                 const float alpha = grow_max ? exp2f((m_used - m_new) * sl) : 1.f;
                 if (grow_max) m_used = m_new;
@@ -601,18 +681,16 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 for (int c4 = 0; c4 < D / 32; ++c4) {
                     uint32_t o[32];
                     tmem_ld32(o_addr + c4 * 32, o);
-                    tmem_ld_wait();
+                    tmem_ld_wait(o);
 #pragma unroll
                     for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
                     tmem_st32(o_addr + c4 * 32, o);
                 }
             }
             const float msl = (m_used == -INFINITY) ? 0.f : m_used * sl;
-            // P = 2^(s*sl - m*sl), two columns at a time.  (Moving a share of the exp2 to the FMA pipe
-            // with a polynomial was measured slower at every share: with one softmax warp per
-            // scheduler and query tile the loop is issue-bound, not MUFU-bound.)
+            // two columns at a time (FFMA2 / FADD2)
             const uint64_t sl2 = pk2(sl, sl), nmsl2 = pk2(-msl, -msl);
-            uint64_t rs2[2] = {0ull, 0ull};                     // (0.f, 0.f)
+            uint64_t rs2[2] = {0ull, 0ull};                         // (0.f, 0.f)
 #pragma unroll
             for (int c = 0; c < kTN / 2; ++c) {
                 uint64_t x = fma2(pk2(__uint_as_float(sv[2 * c]), __uint_as_float(sv[2 * c + 1])), sl2, nmsl2);
@@ -622,7 +700,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 p1 = exp2f(p1);
                 x = pk2(p0, p1);
                 rs2[c & 1] = add2(rs2[c & 1], x);
-                sv[c] = pack_bf16(p0, p1);                      // in place: c <= 2c
+                sv[c] = pack_bf16(p0, p1);                          // in place: c <= 2c
             }
             {
                 float a0, a1, b0, b1;
@@ -631,8 +709,9 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 l_run += (a0 + a1) + (b0 + b1);
             }
             tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&sv[0]));
-            tmem_st32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[32]));
+            if (ncols > 64) tmem_st32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[32]));
             tmem_st_wait();
+            if (threadIdx.x == 128 && jj == 3) TL(57);
             tc_fence_before();
             mbar_arrive(bar_p + 8 * m);
             if (threadIdx.x == 128 && jj < 12) TL(4 + 2 * jj);
@@ -655,7 +734,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 for (int c4 = 0; c4 < D / 32; ++c4) {
                     uint32_t o[32];
                     tmem_ld32(o_addr + c4 * 32, o);
-                    tmem_ld_wait();
+                    tmem_ld_wait(o);
                     if (valid) {
 #pragma unroll
                         for (int q4 = 0; q4 < 4; ++q4) {
@@ -675,7 +754,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 for (int c4 = 0; c4 < D / 32; ++c4) {
                     uint32_t o[32];
                     tmem_ld32(o_addr + c4 * 32, o);
-                    tmem_ld_wait();
+                    tmem_ld_wait(o);
                     if (valid) {
 #pragma unroll
                         for (int q4 = 0; q4 < 8; ++q4)
@@ -697,142 +776,149 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     }
 
     // ---- split-KV combine (a7), in kernel.  The CTAs of one (query tile pair, head) form a
-    //      thread-block cluster, one CTA per split.  Each CTA is responsible for a slice of the
-    //      pair's rows: every CTA sends the other CTAs' slices of its unnormalised partial
-    //      (m, l, O) straight from TMEM into their shared memory (DSMEM), and merges what it
-    //      receives in split order, so the result does not depend on timing. ----
+    //      thread-block cluster, one CTA per split, and each CTA is responsible for a slice of the
+    //      pair's rows.  A CTA writes its partial into its own shared memory, one row per query row:
+    //      O scaled by a power of two 2^-e chosen per row so that the largest element lands in
+    //      [8192, 16384), rounded to fp16 (11 significant bits whatever the magnitude of V), and the
+    //      pair (A, L) = (m + e, l * 2^-e), so that out = sum_s 2^A_s O16_s / sum_s 2^A_s L_s.  The
+    //      TMA engine then copies each peer's slice into that peer's shared memory (one bulk copy per
+    //      peer for O, one for (A, L), completing on the peer's mbarrier), and every CTA merges what it
+    //      received in split order, so the result does not depend on timing. ----
     if (a.cluster_combine) {
-        constexpr int CH = D / 4;                                  // 16-byte chunks per fp32 row
-        const int ns = (need_max + a.split_tiles - 1) / a.split_tiles;     // CTAs that hold keys
+        constexpr int CH = D / 8;                                  // 16-byte units per fp16 row
         const int nrows = min(kPairM, n_s - tok0);
-        const int per = (nrows + ns - 1) / ns;                     // rows per CTA
-        const uint32_t recv_o = ring, recv_ml = ring + (kPairM + 16) * D * 4;   // [src][per][D] fp32, [src][per] (m, l)
-        cluster_sync_all();                  // every CTA of the cluster is done with its ring
-        if (threadIdx.x == 128) TL(31);
+        const int per = (((nrows + ns_act - 1) / ns_act) + 1) & ~1; // rows per CTA, even: (A, L) slices stay 16-byte units
+        const int r_begin = min(nrows, split * per), n_mine = min(nrows, r_begin + per) - r_begin;
+        const uint32_t stage_o = q_smem, stage_ml = base + P::kMlOff;
+        const uint32_t recv_o = ring, recv_ml = ring + P::kRecvMlOff;
+        if (threadIdx.x == 128)         // arm before any peer can send: everything the other CTAs owe this one
+            mbar_expect_tx(bar_recv, (uint32_t)((ns_act - 1) * (n_mine * P::kRowB + ((n_mine + 1) & ~1) * 8)));
+        cluster_arrive();               // this CTA's ring is free (softmax threads arrive after the last MMA)
         if (warp >= 4) {
             const int m = (warp - 4) >> 2, wl = warp & 3;
             const int prow = m * kTM + wl * 32 + lane;             // row of the pair
-            const bool valid = prow < nrows;
-            const int dst = valid ? prow / per : 0, i = prow - dst * per;
-            const uint32_t slot = (uint32_t)(split * per + i);
-            uint32_t rem_o, rem_ml;
-            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rem_o) : "r"(recv_o + slot * (D * 4)), "r"(dst));
-            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rem_ml) : "r"(recv_ml + slot * 8), "r"(dst));
-            if (valid)
-                asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" :: "r"(rem_ml), "f"(nt[m] > 0 ? fin_m : -INFINITY),
-                             "f"(nt[m] > 0 ? fin_l : 0.f) : "memory");
+            const uint32_t o_addr = tmem + ((uint32_t)(wl * 32) << 16) + 256 + m * 128;
+            const uint32_t dst_row = stage_o + (uint32_t)prow * P::kRowB;
             if (nt[m] > 0) {
-                // O rows go out through a per-warp 32 x 128-byte transposing scratch (in the idle Q
-                // area), so that a remote store instruction writes four 128-byte runs instead of
-                // 32 isolated 16-byte pieces.  Within a 128-byte run the 16-byte chunks are XORed
-                // with (row & 7) -- conflict-free for the row-per-thread writes, and the same
-                // order in the scratch and at the destination, so the read-out is a linear copy.
-                const uint32_t o_addr = tmem + ((uint32_t)(wl * 32) << 16) + 256 + m * 128;
-                const uint32_t scratch = q_smem + (uint32_t)(warp - 4) * 4096;
-                uint32_t rem_row[8];                               // destination row of (it*4 + lane/8)
-                bool ok_row[8];
-#pragma unroll
-                for (int it = 0; it < 8; ++it) {
-                    const int pr = m * kTM + wl * 32 + it * 4 + (lane >> 3);
-                    ok_row[it] = pr < nrows;
-                    const int d = ok_row[it] ? pr / per : 0, ii = pr - d * per;
-                    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rem_row[it])
-                                 : "r"(recv_o + (uint32_t)(split * per + ii) * (D * 4) + (lane & 7) * 16), "r"(d));
-                }
+                float amax = 0.f;
 #pragma unroll
                 for (int c4 = 0; c4 < D / 32; ++c4) {
                     uint32_t o[32];
                     tmem_ld32(o_addr + c4 * 32, o);
-                    tmem_ld_wait();
-                    __syncwarp();                                  // previous read-out of the scratch is done
+                    tmem_ld_wait(o);
 #pragma unroll
-                    for (int q = 0; q < 8; ++q)
+                    for (int c = 0; c < 32; c += 2)
+                        amax = max3(amax, fabsf(__uint_as_float(o[c])), fabsf(__uint_as_float(o[c + 1])));
+                }
+                // 2^e = the power of two that brings amax into [8192, 16384); all-zero rows keep e = 0
+                int e = (int)((__float_as_uint(amax) >> 23) & 0xffu) - 140;
+                e = amax > 0.f ? max(e, -100) : 0;
+                const float scale = __uint_as_float((uint32_t)(127 - e) << 23);       // 2^-e
+                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(stage_ml + (uint32_t)prow * 8),
+                             "f"(fin_m + (float)e), "f"(fin_l * scale) : "memory");
+#pragma unroll
+                for (int c4 = 0; c4 < D / 32; ++c4) {
+                    uint32_t o[32];
+                    tmem_ld32(o_addr + c4 * 32, o);
+                    tmem_ld_wait(o);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {                  // 8 values = one 16-byte unit
+                        const uint32_t u = (uint32_t)((c4 * 4 + q) ^ (prow & (CH - 1)));
                         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
-                                     :: "r"(scratch + lane * 128 + (((uint32_t)q ^ (lane & 7)) << 4)), "r"(o[q * 4]), "r"(o[q * 4 + 1]),
-                                        "r"(o[q * 4 + 2]), "r"(o[q * 4 + 3]) : "memory");
-                    __syncwarp();
-#pragma unroll
-                    for (int it = 0; it < 8; ++it) {
-                        uint32_t x, y, z, w;
-                        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(w)
-                                     : "r"(scratch + it * 512 + lane * 16));
-                        if (ok_row[it])
-                            asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};"
-                                         :: "r"(rem_row[it] + c4 * 128), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+                                     :: "r"(dst_row + (u << 4)),
+                                        "r"(pack_f16(__uint_as_float(o[q * 8 + 0]) * scale, __uint_as_float(o[q * 8 + 1]) * scale)),
+                                        "r"(pack_f16(__uint_as_float(o[q * 8 + 2]) * scale, __uint_as_float(o[q * 8 + 3]) * scale)),
+                                        "r"(pack_f16(__uint_as_float(o[q * 8 + 4]) * scale, __uint_as_float(o[q * 8 + 5]) * scale)),
+                                        "r"(pack_f16(__uint_as_float(o[q * 8 + 6]) * scale, __uint_as_float(o[q * 8 + 7]) * scale))
+                                     : "memory");
                     }
                 }
+            } else {
+                // the tile sees none of this split's keys: weight 0 (its O row is never read)
+                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(stage_ml + (uint32_t)prow * 8),
+                             "f"(-INFINITY), "f"(0.f) : "memory");
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // these stores -> the TMA engine's reads
+            asm volatile("bar.sync 1, 256;" ::: "memory");                 // the 8 softmax warps
+        }
+        if (threadIdx.x == 128) TL(31);
+        cluster_wait();                 // every CTA of the cluster is done with its ring and has armed its barrier
+        if (threadIdx.x == 128) {
+            for (int d = 1; d < ns_act; ++d) {                     // start with the next CTA: spreads the traffic
+                const int dst = (split + d) % ns_act;
+                const int d_begin = min(nrows, dst * per), n_dst = min(nrows, d_begin + per) - d_begin;
+                if (n_dst <= 0) continue;
+                const uint32_t pbar = mapa(bar_recv, dst);
+                bulk_s2peer(mapa(recv_o + (uint32_t)(split * per) * P::kRowB, dst), stage_o + (uint32_t)d_begin * P::kRowB,
+                            (uint32_t)n_dst * P::kRowB, pbar);
+                bulk_s2peer(mapa(recv_ml + (uint32_t)(split * per) * 8, dst), stage_ml + (uint32_t)d_begin * 8,
+                            (uint32_t)((n_dst + 1) & ~1) * 8, pbar);
             }
         }
-        if (threadIdx.x == 128) TL(32);
-        cluster_sync_all();                  // all partials have landed
-        if (threadIdx.x == 128) TL(34);
         if (warp >= 4) {
+            mbar_wait_cluster(bar_recv, 0);
+            if (threadIdx.x == 128) TL(32);
+        }
+        cluster_arrive();               // what this CTA had to receive has landed (so its senders' reads are done)
+        if (warp >= 4 && n_mine > 0) {
             constexpr int RW = 32 / CH;                            // rows a warp handles per step
-            constexpr int RB = 4;                                  // steps in flight
-            const int w8 = warp - 4, pch = lane % CH;
-            const int r_begin = split * per, n_mine = min(nrows, r_begin + per) - r_begin;
-            for (int i0 = w8 * RW + lane / CH; i0 < n_mine; i0 += 8 * RW * RB) {
-                float Mrow[RB];
-                // all loads first (unconditional: a split that sent no O leaves stale but unused bytes)
-                float2 ml[RB][4];
-                float4 v[RB][4];
-                float4 acc[RB];
-                float W[RB];
+            const int w8 = warp - 4, u = lane % CH;
+            for (int i = w8 * RW + lane / CH; i < n_mine; i += 8 * RW) {
+                const int prow = r_begin + i;
+                // split sp's partial of this row: own slice from the staging area, the others as received
+                auto ml_addr = [&](int sp) {
+                    return sp == split ? stage_ml + (uint32_t)prow * 8 : recv_ml + (uint32_t)(sp * per + i) * 8;
+                };
+                auto o_addr_of = [&](int sp) {
+                    return (sp == split ? stage_o + (uint32_t)prow * P::kRowB : recv_o + (uint32_t)(sp * per + i) * P::kRowB) +
+                           ((uint32_t)u << 4);
+                };
+                float Amax = -INFINITY;
+                for (int sp = 0; sp < ns_act; ++sp) {
+                    float A;
+                    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(A) : "r"(ml_addr(sp)));
+                    Amax = fmaxf(Amax, A);
+                }
+                float acc[8], W = 0.f;
 #pragma unroll
-                for (int k = 0; k < RB; ++k) { acc[k] = make_float4(0.f, 0.f, 0.f, 0.f); W[k] = 0.f; }
+                for (int k = 0; k < 8; ++k) acc[k] = 0.f;
+                for (int sp0 = 0; sp0 < ns_act; sp0 += 4) {        // splits in order, four loads in flight
+                    float A[4], L[4];
+                    uint4 v[4];
 #pragma unroll
-                for (int sp0 = 0; sp0 < kMaxCluster; sp0 += 4) { // splits in order, four at a time
-                    if (sp0 >= ns) break;
-#pragma unroll
-                    for (int k = 0; k < RB; ++k) {
-                        const int i = min(i0 + k * 8 * RW, n_mine - 1);   // clamped duplicates are not written
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const int sp = min(sp0 + q, ns - 1);
-                            asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(ml[k][q].x), "=f"(ml[k][q].y)
-                                         : "r"(recv_ml + (uint32_t)(sp * per + i) * 8));
-                            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
-                                         : "=f"(v[k][q].x), "=f"(v[k][q].y), "=f"(v[k][q].z), "=f"(v[k][q].w)
-                                         : "r"(recv_o + (uint32_t)(sp * per + i) * (D * 4) + pch * 16));
-                            if (sp0 + q >= ns) ml[k][q] = make_float2(-INFINITY, 0.f);
-                        }
+                    for (int q = 0; q < 4; ++q) {
+                        const int sp = min(sp0 + q, ns_act - 1);
+                        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(A[q]), "=f"(L[q]) : "r"(ml_addr(sp)));
+                        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                                     : "=r"(v[q].x), "=r"(v[q].y), "=r"(v[q].z), "=r"(v[q].w) : "r"(o_addr_of(sp)));
+                        if (sp0 + q >= ns_act) A[q] = -INFINITY;
                     }
-                    // merge this group into the running (M, W, acc) of each row: the running max
-                    // is the first group's max unless a later group raises it (rescale, rare)
 #pragma unroll
-                    for (int k = 0; k < RB; ++k) {
-                        float Mg = fmaxf(fmaxf(ml[k][0].x, ml[k][1].x), fmaxf(ml[k][2].x, ml[k][3].x));
-                        if (sp0 == 0) Mrow[k] = Mg;
-                        else if (Mg > Mrow[k]) {
-                            const float sc = exp2f(Mrow[k] - Mg);   // Mrow finite or -inf (then sc = 0 and acc = 0)
-                            acc[k].x *= sc; acc[k].y *= sc; acc[k].z *= sc; acc[k].w *= sc; W[k] *= sc;
-                            Mrow[k] = Mg;
-                        }
+                    for (int q = 0; q < 4; ++q) {
+                        const bool on = A[q] != -INFINITY;         // a split that sent no O leaves stale but unused bytes
+                        const float wgt = on ? exp2f(A[q] - Amax) : 0.f;
+                        W += on ? wgt * L[q] : 0.f;
+                        const uint32_t w4[4] = {v[q].x, v[q].y, v[q].z, v[q].w};
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const bool on = ml[k][q].x != -INFINITY;
-                            const float wgt = on ? exp2f(ml[k][q].x - Mrow[k]) : 0.f;
-                            W[k] += wgt * ml[k][q].y;
-                            acc[k].x += on ? wgt * v[k][q].x : 0.f; acc[k].y += on ? wgt * v[k][q].y : 0.f;
-                            acc[k].z += on ? wgt * v[k][q].z : 0.f; acc[k].w += on ? wgt * v[k][q].w : 0.f;
+                        for (int k = 0; k < 4; ++k) {
+                            const float2 f = unpack_f16(w4[k]);
+                            acc[2 * k] += on ? wgt * f.x : 0.f;
+                            acc[2 * k + 1] += on ? wgt * f.y : 0.f;
                         }
                     }
                 }
-#pragma unroll
-                for (int k = 0; k < RB; ++k) {
-                    const int i = i0 + k * 8 * RW;
-                    if (i >= n_mine) continue;
-                    const int prow = r_begin + i;
-                    const float inv = __fdividef(1.f, W[k]);
-                    uint2 o2;
-                    o2.x = pack_bf16(acc[k].x * inv, acc[k].y * inv);
-                    o2.y = pack_bf16(acc[k].z * inv, acc[k].w * inv);
-                    const int64_t grow = (int64_t)b.cu_new[s] + tok0 + prow;
-                    const int c = (pch & ~7) | ((pch & 7) ^ (prow & 7));   // un-swizzle: which columns this chunk holds
-                    *reinterpret_cast<uint2 *>((char *)a.out + (grow * g.Hq + h) * (D * 2) + c * 8) = o2;
-                }
+                const float inv = __fdividef(1.f, W);
+                uint4 o4;
+                o4.x = pack_bf16(acc[0] * inv, acc[1] * inv);
+                o4.y = pack_bf16(acc[2] * inv, acc[3] * inv);
+                o4.z = pack_bf16(acc[4] * inv, acc[5] * inv);
+                o4.w = pack_bf16(acc[6] * inv, acc[7] * inv);
+                const int64_t grow = (int64_t)b.cu_new[s] + tok0 + prow;
+                const int c = u ^ (prow & (CH - 1));               // un-swizzle: which 8 columns this unit holds
+                *reinterpret_cast<uint4 *>((char *)a.out + (grow * g.Hq + h) * (D * 2) + c * 16) = o4;
             }
         }
+        cluster_wait();                 // no CTA leaves while a peer's copy may still read its shared memory
     }
 
     if (threadIdx.x == 128) { TL(33); TLG(61); }
@@ -845,7 +931,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 }  // namespace
 
 int sc_tc_tile_m() { return kPairM; }
-int sc_tc_tile_n() { return kTN; }
+int sc_tc_split_unit() { return 16; }          // splits are in pool blocks
 
 template <int D, int LEAN>
 static cudaError_t prepare_tc()
@@ -859,7 +945,7 @@ static cudaError_t prepare_tc()
 }
 
 template <int D, int LEAN>
-static void fill_config(cudaLaunchConfig_t &cfg, cudaLaunchAttribute *attr, dim3 grid, int cluster, cudaStream_t st)
+static void fill_config(cudaLaunchConfig_t &cfg, cudaLaunchAttribute *attr, dim3 grid, int cluster, bool pdl, cudaStream_t st)
 {
     cfg = cudaLaunchConfig_t{};
     cfg.gridDim = grid;
@@ -870,8 +956,12 @@ static void fill_config(cudaLaunchConfig_t &cfg, cudaLaunchAttribute *attr, dim3
     attr[0].val.clusterDim.x = cluster;                               // one CTA per split
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    // Programmatic dependent launch: this kernel may be scheduled while the kernel before it in the
+    // stream drains; it waits (griddepcontrol.wait) before it touches anything that kernel wrote.
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = pdl ? 2 : 1;
 }
 
 template <int D, int LEAN>
@@ -880,8 +970,8 @@ static cudaError_t launch_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs
     cudaError_t e = prepare_tc<D, LEAN>();
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg;
-    cudaLaunchAttribute attr[1];
-    fill_config<D, LEAN>(cfg, attr, grid, a.cluster_combine ? (int)grid.x : 1, st);
+    cudaLaunchAttribute attr[2];
+    fill_config<D, LEAN>(cfg, attr, grid, a.cluster_combine ? (int)grid.x : 1, a.pdl != 0, st);
     return cudaLaunchKernelEx(&cfg, sc_attn_tc_kernel<D, LEAN>, g, b, a);
 }
 
@@ -892,8 +982,8 @@ static int wave_ctas(int cluster)
 {
     if (prepare_tc<D, LEAN>() != cudaSuccess) return 0;
     cudaLaunchConfig_t cfg;
-    cudaLaunchAttribute attr[1];
-    fill_config<D, LEAN>(cfg, attr, dim3((unsigned)cluster, 1, 1), cluster, nullptr);
+    cudaLaunchAttribute attr[2];
+    fill_config<D, LEAN>(cfg, attr, dim3((unsigned)cluster, 1, 1), cluster, false, nullptr);
     int n = 0;
     if (cudaOccupancyMaxActiveClusters(&n, sc_attn_tc_kernel<D, LEAN>, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
     return n * cluster;

@@ -34,30 +34,50 @@ __device__ __forceinline__ int seq_of(const int32_t *cu, int n_seq, int x)
 }
 
 // ------------------------------------------------------------ scatter / read
-// One thread per 16 bytes (8 bf16 of one head of one token, K or V).
+// One thread per 16 bytes (8 bf16 of one head of one token, K or V).  The scatter (kToPool) has
+// `pad` != 0 when it stores a turn's new tokens: after the n_units data units come, per sequence,
+// the 15 slots that may follow its last token inside the last block, and those that exist are
+// zero-filled -- slots past the logical end then hold finite values whatever the memory held
+// before (attention masks them in S, but 0 * NaN in P.V would poison the row).
 template <bool kToPool>
 __global__ void __launch_bounds__(256)
 sc_scatter_read_kernel(ScGeom g, ScBatch b, char *k_lin, char *v_lin, ScKvView view0,
-                       ScKvView view1, int has_view1, int64_t n_units)
+                       ScKvView view1, int has_view1, int64_t n_units, int pad)
 {
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= n_units) return;
+    int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int cpr = g.D >> 3;                       // 16-byte units per head row
     const int c = (int)(idx % cpr);
     int64_t t = idx / cpr;
     const int h = (int)(t % g.Hkv);
     t /= g.Hkv;
-    const int total = b.cu_new[b.n_seq];
-    const int row = (int)(t % total);
-    const int kv = (int)(t / total);
-    const int s = seq_of(b.cu_new, b.n_seq, row);
-    const int tok = b.hist[s] + (row - b.cu_new[s]);
+    int s, tok, kv;
+    int64_t row = 0;
+    bool zero = false;
+    if (idx < n_units) {
+        const int total = b.cu_new[b.n_seq];
+        row = t % total;
+        kv = (int)(t / total);
+        s = seq_of(b.cu_new, b.n_seq, (int)row);
+        tok = b.hist[s] + ((int)row - b.cu_new[s]);
+    } else {
+        if (!kToPool || !pad) return;
+        t -= (int64_t)b.cu_new[b.n_seq] * 2;        // (kv, sequence, slot after the end) past the data rows
+        const int p = (int)(t % 15);
+        t /= 15;
+        s = (int)(t % b.n_seq);
+        kv = (int)(t / b.n_seq);
+        if (kv > 1) return;
+        const int end = b.hist[s] + (b.cu_new[s + 1] - b.cu_new[s]);
+        if (b.cu_new[s + 1] == b.cu_new[s] || (end & 15) == 0 || (end & 15) + p > 15) return;
+        tok = end + p;
+        zero = true;
+    }
     const int lb = tok >> 4, slot = tok & 15;
-    char *lin = (kv ? v_lin : k_lin) + (((int64_t)row * g.Hkv + h) * g.D + c * 8) * 2;
+    char *lin = (kv ? v_lin : k_lin) + ((row * g.Hkv + h) * g.D + c * 8) * 2;
     const int64_t in_cell = (int64_t)(kv * g.Hkv + h) * g.chunk_bytes + sc_chunk_off(slot, c * 8, g.nh);
     char *p0 = view0.base + sc_phys_block(view0, b, s, lb) * view0.block_stride + in_cell;
     if (kToPool) {
-        const int4 val = ld_stream(lin);
+        const int4 val = zero ? make_int4(0, 0, 0, 0) : ld_stream(lin);
         *reinterpret_cast<int4 *>(p0) = val;
         if (has_view1) {
             char *p1 = view1.base + sc_phys_block(view1, b, s, lb) * view1.block_stride + in_cell;
@@ -189,13 +209,15 @@ sc_gather_bulk_kernel(ScGeom g, ScBatch b, ScKvView src, ScKvView dst, int piece
 
 // ------------------------------------------------------------------ launchers
 cudaError_t sc_launch_scatter(const ScGeom &g, const void *k, const void *v, const ScBatch &b,
-                              const ScKvView &dst0, const ScKvView *dst1, cudaStream_t st)
+                              const ScKvView &dst0, const ScKvView *dst1, bool pad_last_block, cudaStream_t st)
 {
-    const int64_t units = (int64_t)b.cu_new[b.n_seq] * 2 * g.Hkv * (g.D / 8);
+    const int64_t per_row = (int64_t)g.Hkv * (g.D / 8);
+    const int64_t units = (int64_t)b.cu_new[b.n_seq] * 2 * per_row;
     if (units == 0) return cudaSuccess;
-    const unsigned grid = (unsigned)((units + 255) / 256);
+    const int64_t pad_units = pad_last_block ? (int64_t)b.n_seq * 2 * 15 * per_row : 0;
+    const unsigned grid = (unsigned)((units + pad_units + 255) / 256);
     sc_scatter_read_kernel<true><<<grid, 256, 0, st>>>(g, b, (char *)k, (char *)v, dst0,
-                                                        dst1 ? *dst1 : dst0, dst1 != nullptr, units);
+                                                        dst1 ? *dst1 : dst0, dst1 != nullptr, units, pad_last_block);
     return cudaGetLastError();
 }
 
@@ -206,7 +228,7 @@ cudaError_t sc_launch_read(const ScGeom &g, void *k_out, void *v_out, const ScBa
     if (units == 0) return cudaSuccess;
     const unsigned grid = (unsigned)((units + 255) / 256);
     sc_scatter_read_kernel<false><<<grid, 256, 0, st>>>(g, b, (char *)k_out, (char *)v_out, src, src,
-                                                         0, units);
+                                                         0, units, 0);
     return cudaGetLastError();
 }
 

@@ -136,7 +136,7 @@ constexpr int SC_MAX_DEVICES = 64;
 // ------------------------------------------------------- kernel launchers
 // sc_copy.cu
 cudaError_t sc_launch_scatter(const ScGeom &g, const void *k, const void *v, const ScBatch &b,
-                              const ScKvView &dst0, const ScKvView *dst1, cudaStream_t st);
+                              const ScKvView &dst0, const ScKvView *dst1, bool pad_last_block, cudaStream_t st);
 cudaError_t sc_launch_read(const ScGeom &g, void *k_out, void *v_out, const ScBatch &b,
                            const ScKvView &src, cudaStream_t st);
 cudaError_t sc_launch_gather(const ScGeom &g, const ScBatch &b, const ScKvView &src,
@@ -155,18 +155,20 @@ struct ScAttnArgs {
     ScKvView scat0, scat1;       // where to scatter: the pool, and (staged mode) the LSC
     int32_t has_scat1;
     int32_t cluster_combine;  // tcgen05 engine: the splits of a query tile group form a cluster and merge in kernel
-    int32_t split_tiles;  // KV tiles per split
+    int32_t pdl;          // tcgen05 engine: launch with programmatic stream serialization
+    int32_t split_units;  // KV units per split; a unit is the engine's split granule in tokens
+                          // (sc_mma_split_unit(): its 64-token tile; sc_tc_split_unit(): a 16-token pool block)
     int32_t n_splits;     // grid extent over splits (max over rows)
     int32_t total_new;    // sum n
 };
-int sc_mma_tile_m();   // query rows per CTA of the mma.sync engine
-int sc_mma_tile_n();   // KV tokens per tile
+int sc_mma_tile_m();       // query rows per CTA of the mma.sync engine
+int sc_mma_split_unit();   // tokens per split unit (its KV tile)
 cudaError_t sc_launch_attn_mma(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st);
 // sc_attn_tc.cu  (tcgen05 / TMEM engine): a CTA owns a pair of 128-row query tiles
 int sc_tc_tile_m();
-int sc_tc_tile_n();
+int sc_tc_split_unit();    // tokens per split unit (a pool block)
 int sc_tc_max_cluster();   // most splits the in-kernel (cluster) combine handles
 int sc_tc_wave_ctas(int D, int lean, int cluster);   // co-resident CTAs when launched in clusters of that size
 cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st);
 cudaError_t sc_launch_combine(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, int tile_m,
-                              int tile_n, cudaStream_t st);
+                              int split_unit, cudaStream_t st);

@@ -85,62 +85,57 @@ sc_status_t make_batch(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, 
 
 int lsc_blocks_needed(const ScBatch &b) { return b.lsc_total; }
 
-// KV tiles per split.  Every (query tile group, head) needs ceil(tiles/split) CTAs of up to
-// `split` tiles each; the grid runs in waves of n_sms*ctas_per_sm CTAs, and a CTA costs its
-// tiles plus a fixed overhead (prologue, epilogue, partial write + combine read).  Pick the
-// split with the smallest  waves * (split + overhead).  Depends on logical lengths only.
-// KV tiles per split, and whether the splits of a query pair run as one thread-block cluster.
-// Every (query tile group, head) needs ceil(tiles/split) CTAs of up to `split` tiles each; the
-// grid runs in waves, and a CTA costs its tiles plus a fixed overhead (prologue, epilogue).
-// Costs are in units of one KV tile (~1.9 us on B200), fitted to measurements:
+// How the KV range of a batch is split over CTAs.  Splits are counted in the engine's split unit
+// (tcgen05: a 16-token pool block, so that e.g. 336 blocks over 4 CTAs are 84 each = 10.5 KV tiles;
+// mma.sync: its 64-token tile).  Every (query tile group, head) needs ceil(units/split) CTAs; the
+// grid runs in waves, and a CTA costs its KV tiles plus a fixed overhead (prologue, epilogue).
+// Costs are in units of one 128-token KV tile (~1.8 us on B200), fitted to measurements:
 //   cluster (tcgen05, <= 16 splits, ONE wave only -- clusters of whole-SM CTAs place badly over
-//            several waves -- and <= 128 tiles per CTA): in-kernel scatter + DSMEM combine, ~4
+//            several waves -- and <= 128 tiles per CTA): in-kernel scatter + DSMEM combine, ~3
 //   plain  : separate scatter (~5) and combine (~1.3 per split) kernels, partial write ~2 per wave
 // Depends on logical lengths only.
-struct SplitChoice { int split_tiles; bool cluster; };
+struct SplitChoice { int split_units; bool cluster; };
 
-SplitChoice choose_split_tiles(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, const int32_t *cu_new,
-                               int tile_m, int tile_n, bool tc, bool staged)
+SplitChoice choose_split(const sc_pool_t *p, int n_seq, const int32_t *hist_lens, const int32_t *cu_new,
+                         int tile_m, int unit, bool tc, bool staged)
 {
-    int max_tiles = 1;
+    int max_units = 1;
     for (int i = 0; i < n_seq; ++i)
-        max_tiles = std::max(max_tiles, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), tile_n));
-    SplitChoice best = {max_tiles, false};
+        max_units = std::max(max_units, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), unit));
+    const double units_per_tile = 128.0 / unit;
+    SplitChoice best = {max_units, false};
     double best_cost = 1e30;
     for (int n_sp = 1; n_sp <= p->max_splits; ++n_sp) {
-        const int split = ceil_div(max_tiles, n_sp);
-        if (n_sp > 1 && ceil_div(max_tiles, split) != n_sp) continue;     // same split as a smaller n_sp
+        const int split = ceil_div(max_units, n_sp);
+        if (n_sp > 1 && ceil_div(max_units, split) != n_sp) continue;     // same split as a smaller n_sp
         int64_t ctas = 0;
         for (int i = 0; i < n_seq; ++i) {
             const int n = cu_new[i + 1] - cu_new[i];
             for (int mt = 0; mt * tile_m < n; ++mt) {
                 const int kmax = hist_lens[i] + std::min(n, (mt + 1) * tile_m);
-                ctas += (int64_t)p->g.Hq * ceil_div(ceil_div(kmax, tile_n), split);
+                ctas += (int64_t)p->g.Hq * ceil_div(ceil_div(kmax, unit), split);
             }
         }
         for (int use_cluster = 0; use_cluster < 2; ++use_cluster) {
             int64_t wave = (int64_t)p->n_sms * (tc ? 1 : 3);
             double extra = 0.0;
             if (use_cluster) {
-                if (!tc || n_sp < 2 || n_sp > sc_tc_max_cluster() || split > 128) continue;
+                if (!tc || n_sp < 2 || n_sp > sc_tc_max_cluster() || split > 128 * units_per_tile) continue;
                 wave = sc_tc_wave_ctas(p->g.D, staged, n_sp);
                 // the launch is n_sp CTAs per (pair, head) whether or not a sequence needs them all
                 int64_t launched = 0;
                 for (int i = 0; i < n_seq; ++i)
                     launched += (int64_t)p->g.Hq * ceil_div(cu_new[i + 1] - cu_new[i], tile_m) * n_sp;
                 if (wave <= 0 || launched > wave) continue;
-                extra = 4.0;
+                extra = 3.0;
             }
             const double waves = (double)((ctas + wave - 1) / wave);
             if (!use_cluster && n_sp > 1) extra = (tc ? 5.0 : 0.5) + 1.3 * n_sp + 2.0 * waves;
-            const double cost = waves * (split + 3.0) + extra;
-#ifdef SC_TC_PROBE
-            if (getenv("SC_DEBUG_SPLIT")) fprintf(stderr, "n_sp %d cluster %d split %d ctas %lld wave %lld waves %.0f cost %.1f\n", n_sp, use_cluster, split, (long long)ctas, (long long)wave, waves, cost);
-#endif
+            const double cost = waves * (split / units_per_tile + 3.0) + extra;
             if (cost < best_cost - 1e-9) { best_cost = cost; best = {split, use_cluster != 0}; }
         }
     }
-    best.split_tiles = std::max(best.split_tiles, 1);
+    best.split_units = std::max(best.split_units, 1);
     return best;
 }
 
@@ -167,7 +162,7 @@ sc_status_t sc_store_prefix(sc_pool_t *pool, int32_t layer, const void *k, const
     b.cu_new[1] = n_tokens;
     {
         ScProfScope ps(pool, SC_KERNEL_SCATTER, (cudaStream_t)stream);
-        SC_CUDA(sc_launch_scatter(pool->g, k, v, b, pool_view(pool, layer, table_dev, n_table), nullptr,
+        SC_CUDA(sc_launch_scatter(pool->g, k, v, b, pool_view(pool, layer, table_dev, n_table), nullptr, false,
                                   (cudaStream_t)stream));
     }
     pool->launches += 1;
@@ -256,7 +251,7 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     int engine = pool->attn_engine;
     if (engine == SC_ENGINE_AUTO) engine = SC_ENGINE_TCGEN05;
     const bool tc = (engine == SC_ENGINE_TCGEN05);
-    const int tile_m = tc ? sc_tc_tile_m() : sc_mma_tile_m(), tile_n = tc ? sc_tc_tile_n() : sc_mma_tile_n();
+    const int tile_m = tc ? sc_tc_tile_m() : sc_mma_tile_m(), unit = tc ? sc_tc_split_unit() : sc_mma_split_unit();
     ScBatch b;
     st = make_batch(pool, n_seq, hist_lens, cu_new, max_blocks, tile_m, &b);
     if (st) return st;
@@ -266,29 +261,34 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     if (staged && (!pool->lsc_base || lsc_blocks_needed(b) > pool->cfg.lsc_blocks))
         return sc_fail(SC_ERR_CAPACITY, "batch needs %d LSC blocks, buffer holds %d", lsc_blocks_needed(b),
                        pool->cfg.lsc_blocks);
+    const bool has_res = staged && pool->resident_blocks > 0;
+    if (has_res && !tc)          // checked before the first launch: an error leaves pool and LSC untouched
+        return sc_fail(SC_ERR_UNSUPPORTED, "resident blocks in staged mode need the tcgen05 engine");
     cudaStream_t s = (cudaStream_t)stream;
     const ScKvView pv = pool_view(pool, layer, tables_dev, max_blocks);
     const ScKvView lv = staged ? lsc_view(pool, buf) : pv;
 
     // split of the KV range over CTAs, when that is needed to fill the machine
-    int split_tiles = pool->split_tiles_override;
     bool cluster = false;
-    int max_tiles = 1;
+    int max_units = 1;
     for (int i = 0; i < n_seq; ++i)
-        max_tiles = std::max(max_tiles, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), tile_n));
-    if (split_tiles <= 0) {
-        const SplitChoice c = choose_split_tiles(pool, n_seq, hist_lens, cu_new, tile_m, tile_n, tc, staged);
-        split_tiles = c.split_tiles;
+        max_units = std::max(max_units, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), unit));
+    int split_units;
+    if (pool->split_tiles_override <= 0) {
+        const SplitChoice c = choose_split(pool, n_seq, hist_lens, cu_new, tile_m, unit, tc, staged);
+        split_units = c.split_units;
         cluster = c.cluster;
     } else {
-        // forced split (tests, experiments): cluster whenever such a cluster can be placed
-        const int ns = ceil_div(max_tiles, split_tiles);
+        // forced split (tests, experiments), given in KV tiles of the engine (tcgen05: 128 tokens,
+        // mma.sync: 64): cluster whenever such a cluster can be placed
+        split_units = pool->split_tiles_override * (tc ? 128 / unit : 1);
+        const int ns = ceil_div(max_units, split_units);
         cluster = tc && ns > 1 && ns <= sc_tc_max_cluster() && sc_tc_wave_ctas(pool->g.D, staged, ns) > 0;
     }
-    int n_splits = ceil_div(max_tiles, split_tiles);
+    int n_splits = ceil_div(max_units, split_units);
     if (n_splits > pool->max_splits) {
-        split_tiles = ceil_div(max_tiles, pool->max_splits);
-        n_splits = ceil_div(max_tiles, split_tiles);
+        split_units = ceil_div(max_units, pool->max_splits);
+        n_splits = ceil_div(max_units, split_units);
         cluster = false;
     }
     if (n_splits == 1) cluster = false;
@@ -298,7 +298,7 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     const bool fold_scatter = tc && (cluster || n_splits == 1);
     if (!fold_scatter) {
         ScProfScope ps(pool, SC_KERNEL_SCATTER, s);
-        SC_CUDA(sc_launch_scatter(pool->g, k_new, v_new, b, pv, staged ? &lv : nullptr, s));
+        SC_CUDA(sc_launch_scatter(pool->g, k_new, v_new, b, pv, staged ? &lv : nullptr, true, s));
         pool->launches += 1;
     }
 
@@ -312,13 +312,13 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     a.k_new = fold_scatter ? k_new : nullptr;
     a.v_new = fold_scatter ? v_new : nullptr;
     a.kv_res = pv;
-    a.has_res = (staged && pool->resident_blocks > 0) ? 1 : 0;
-    if (a.has_res && !tc) return sc_fail(SC_ERR_UNSUPPORTED, "resident blocks in staged mode need the tcgen05 engine");
+    a.has_res = has_res ? 1 : 0;
     a.scat0 = pv;
     a.scat1 = lv;
     a.has_scat1 = staged ? 1 : 0;
     a.cluster_combine = cluster ? 1 : 0;
-    a.split_tiles = split_tiles;
+    a.pdl = tc ? 1 : 0;
+    a.split_units = split_units;
     a.n_splits = n_splits;
     a.total_new = total_new;
     {
@@ -326,12 +326,12 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
         SC_CUDA(tc ? sc_launch_attn_tc(pool->g, b, a, s) : sc_launch_attn_mma(pool->g, b, a, s));
     }
     pool->launches += 1;
-    // 3. combine (a7): with up to 8 splits the tcgen05 engine merges the partials itself (the
-    //    splits of a query tile group form a thread-block cluster); otherwise a separate kernel
+    // 3. combine (a7): with up to 16 splits in one wave the tcgen05 engine merges the partials itself
+    //    (the splits of a query tile group form a thread-block cluster); otherwise a separate kernel
     if (n_splits > 1 && !a.cluster_combine) {
         {
             ScProfScope ps(pool, SC_KERNEL_COMBINE, s);
-            SC_CUDA(sc_launch_combine(pool->g, b, a, tile_m, tile_n, s));
+            SC_CUDA(sc_launch_combine(pool->g, b, a, tile_m, unit, s));
         }
         pool->launches += 1;
     }
