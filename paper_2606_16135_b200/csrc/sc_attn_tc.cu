@@ -292,9 +292,11 @@ __device__ __forceinline__ int seq_of(const int32_t *cu, int n_seq, int x)
 //   [kQOff]     Q_0, Q_1 (swizzled like K tiles); in the cluster epilogue: this CTA's partial O, one
 //               row-scaled fp16 row of D values per query row, 16-byte units XORed with the row index
 //   [kRingOff]  the KV ring; in the cluster epilogue: what the peers send, [split][row][D] fp16 and,
-//               from kRecvMlOff, [split][row] (A, L)
+//               from kRecvMlOff, [split][row] (A, L); from kMlOff this CTA's own (A, L) per query row
+//               (written only after BOTH query tiles' last MMA: until then the ring is in use)
 //   [kBarOff]   mbarriers, TMEM base
-//   [kMlOff]    this CTA's (A, L) per query row (cluster epilogue)
+// The total stays 1 KiB under the per-SM limit so that a gather CTA of the copy stream (no shared memory
+// of its own, but 1 KiB is reserved per resident CTA) still fits beside an attention CTA in staged mode.
 template <int D>
 struct Plan {
     static constexpr int NH = D / 64;
@@ -306,12 +308,12 @@ struct Plan {
     static constexpr int kQOff = 0;
     static constexpr int kRingOff = 2 * kQTile;
     static constexpr int kRecvMlOff = kRecvRows * kRowB;          // inside the ring
+    static constexpr int kMlOff = kRingOff + kRecvMlOff + kRecvRows * 8;
     static constexpr int kBarOff = kRingOff + kStages * kSlot;
-    static constexpr int kMlOff = kBarOff + 192;
     static constexpr int kSlack = 832;                 // the dynamic window may start this far off a 1 KiB boundary
-    static constexpr int kBytes = kMlOff + kPairM * 8 + kSlack;
-    static_assert(kRecvMlOff + kRecvRows * 8 <= kStages * kSlot, "receive area must fit in the ring");
-    static_assert(kBytes <= 232448, "more than 227 KB of shared memory");
+    static constexpr int kBytes = kBarOff + 192 + kSlack;
+    static_assert(kMlOff + kPairM * 8 <= kBarOff, "receive and staging areas must fit in the ring");
+    static_assert(kBytes <= 232448 - 1024, "no room left for a co-resident gather CTA");
 };
 
 struct Bars {                       // at Plan::kBarOff
@@ -365,6 +367,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) { TL(0); TLG(60); }
+    LAUNCH_BEGIN();
     const uint32_t bar_full = smem_u32(&bars->full[0]), bar_empty = smem_u32(&bars->empty[0]);
     const uint32_t bar_s = smem_u32(&bars->s_ready[0]), bar_p = smem_u32(&bars->p_ready[0]);
     const uint32_t bar_q = smem_u32(&bars->q_ready[0]), bar_scat = smem_u32(&bars->scat_done);
@@ -799,6 +802,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             const int prow = m * kTM + wl * 32 + lane;             // row of the pair
             const uint32_t o_addr = tmem + ((uint32_t)(wl * 32) << 16) + 256 + m * 128;
             const uint32_t dst_row = stage_o + (uint32_t)prow * P::kRowB;
+            float stA = -INFINITY, stL = 0.f;                       // a tile that sees none of this split's keys: weight 0
             if (nt[m] > 0) {
                 float amax = 0.f;
 #pragma unroll
@@ -814,8 +818,8 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                 int e = (int)((__float_as_uint(amax) >> 23) & 0xffu) - 140;
                 e = amax > 0.f ? max(e, -100) : 0;
                 const float scale = __uint_as_float((uint32_t)(127 - e) << 23);       // 2^-e
-                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(stage_ml + (uint32_t)prow * 8),
-                             "f"(fin_m + (float)e), "f"(fin_l * scale) : "memory");
+                stA = fin_m + (float)e;
+                stL = fin_l * scale;
 #pragma unroll
                 for (int c4 = 0; c4 < D / 32; ++c4) {
                     uint32_t o[32];
@@ -833,11 +837,9 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                                      : "memory");
                     }
                 }
-            } else {
-                // the tile sees none of this split's keys: weight 0 (its O row is never read)
-                asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(stage_ml + (uint32_t)prow * 8),
-                             "f"(-INFINITY), "f"(0.f) : "memory");
             }
+            asm volatile("bar.sync 1, 256;" ::: "memory");                 // both query tiles' MMAs are done: the ring is free
+            asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(stage_ml + (uint32_t)prow * 8), "f"(stA), "f"(stL) : "memory");
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // these stores -> the TMA engine's reads
             asm volatile("bar.sync 1, 256;" ::: "memory");                 // the 8 softmax warps
         }
@@ -922,6 +924,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     }
 
     if (threadIdx.x == 128) { TL(33); TLG(61); }
+    LAUNCH_END();
     tc_fence_before();
     __syncthreads();
     if (warp == 2)
@@ -1006,6 +1009,7 @@ int sc_tc_wave_ctas(int D, int lean, int cluster)
 }
 #ifdef SC_TC_PROBE
 extern "C" int sc_probe_read(long long *host) { return (int)cudaMemcpyFromSymbol(host, sc_tl, sizeof(long long) * 256 * 64); }
+extern "C" int sc_probe_read_launches(long long *host) { return (int)cudaMemcpyFromSymbol(host, sc_lt, sizeof(long long) * 256 * 2); }
 #endif
 
 cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st)

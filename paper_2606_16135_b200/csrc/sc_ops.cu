@@ -317,7 +317,9 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     a.scat1 = lv;
     a.has_scat1 = staged ? 1 : 0;
     a.cluster_combine = cluster ? 1 : 0;
-    a.pdl = tc ? 1 : 0;
+    // programmatic dependent launch only in fused mode: in staged mode the early CTAs of the next layer
+    // would sit on SMs that the concurrent gather of the copy stream can use in full
+    a.pdl = (tc && !staged) ? 1 : 0;
     a.split_units = split_units;
     a.n_splits = n_splits;
     a.total_new = total_new;
