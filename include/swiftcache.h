@@ -113,8 +113,10 @@ sc_status_t sc_pool_bytes_required(const sc_pool_config_t *cfg, size_t *pool_byt
 /* pool_base: DEVICE pointer (SC_POOL_HBM) or pinned, device-mapped HOST pointer
  * (SC_POOL_HOST_PINNED), 1024-byte aligned, >= pool_bytes.  lsc_base: DEVICE pointer,
  * 1024-byte aligned, >= lsc_bytes; may be NULL with lsc_blocks == 0 (fused mode only).
- * If zero_fill != 0 both regions are cleared (S10: slots never written must hold
- * finite values).  Passing pool_base == NULL creates a HOST-ONLY pool object: the
+ * If zero_fill != 0 both regions are cleared; this is optional: the data path never
+ * relies on what a slot it did not write holds (S10: the scatter of a turn zero-fills
+ * the rest of the conversation's last block, every other unwritten slot is outside
+ * what attention reads).  Passing pool_base == NULL creates a HOST-ONLY pool object: the
  * allocator / block-table calls work, every data call fails with SC_ERR_CUDA.       */
 sc_status_t sc_pool_create(const sc_pool_config_t *cfg, void *pool_base, size_t pool_bytes,
                            void *lsc_base, size_t lsc_bytes, int32_t zero_fill, sc_pool_t **out);
@@ -185,7 +187,8 @@ sc_status_t sc_load_layer(sc_pool_t *pool, int32_t layer, const int32_t *table_d
  * table_dev: DEVICE int32[n_table] covering hist_len + n_new tokens (sc_append_blocks).
  * Steps, all enqueued on `stream`:
  *   1. scatter k_new/v_new to logical tokens hist_len.. of the pool (and, in STAGED
- *      mode, to the same logical positions of LSC[buf]);
+ *      mode, to the same logical positions of LSC[buf]); the slots of the last block
+ *      past token hist_len + n_new - 1 are set to zero;
  *   2. out[i,h,:] = sum_j softmax_j(q[i,h].K[j,h/G]/sqrt(D)) V[j,h/G,:], j <= hist_len+i,
  *      K/V = [history ; new], bf16 inputs, fp32 accumulation, bf16 output;
  *      STAGED reads LSC[buf] (history must have been loaded there), FUSED reads the

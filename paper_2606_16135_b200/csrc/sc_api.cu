@@ -203,7 +203,10 @@ sc_status_t sc_pool_info(const sc_pool_t *pool, sc_pool_info_t *info)
     info->lsc_buffer_bytes = pool->lsc_buffer_bytes;
     info->lsc_bytes = 2 * pool->lsc_buffer_bytes;
     info->scratch_bytes = pool->scratch_bytes;
-    info->n_free_blocks = (int32_t)pool->free_list.size();
+    {
+        std::lock_guard<std::mutex> lk(const_cast<sc_pool_t *>(pool)->mu);     // the allocator calls are serialised
+        info->n_free_blocks = (int32_t)pool->free_list.size();
+    }
     info->max_splits = pool->max_splits;
     return SC_OK;
 }
@@ -291,6 +294,7 @@ sc_status_t sc_free_blocks(sc_pool_t *pool, const int32_t *ids, int32_t n)
 sc_status_t sc_num_free_blocks(const sc_pool_t *pool, int32_t *n_free)
 {
     if (!pool || !n_free) return sc_fail(SC_ERR_INVALID_ARG, "NULL argument");
+    std::lock_guard<std::mutex> lk(const_cast<sc_pool_t *>(pool)->mu);
     *n_free = (int32_t)pool->free_list.size();
     return SC_OK;
 }

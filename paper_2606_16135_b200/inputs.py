@@ -136,8 +136,13 @@ def make_qkv(n_new: int, T_h: int, Hq: int, Hkv: int, D: int, seed: int, variant
     variant "peaked": q scaled x16 so the scores have std ~4 and the online
         softmax's running-max rescale is exercised.
     variant "adversarial": additionally the last history token and the last
-        new token get keys aligned with the queries' mean direction, so the
-        largest score arrives in the last KV tile / among the new tokens.
+        new token get, per KV head, a key that is the direction of an ACTUAL
+        query row -- the last new token's query of the group's first query
+        head -- scaled so its largest component is 4.  For that row the two
+        planted keys score |q|^2 * 4 / max|q| (hundreds, against a spread of
+        ~+-25 elsewhere): its largest score arrives in the last history tile
+        and again at its own, last, new token.  Other rows see a large score
+        of either sign there.
     """
     q = normal_bf16((n_new, Hq, D), seed + 1)
     kh = normal_bf16((T_h, Hkv, D), seed + 2)
@@ -148,8 +153,8 @@ def make_qkv(n_new: int, T_h: int, Hq: int, Hkv: int, D: int, seed: int, variant
         q = f32_to_bf16_bits(bf16_bits_to_f32(q) * np.float32(16.0))
     if variant == "adversarial":
         G = Hq // Hkv
-        qf = bf16_bits_to_f32(q).reshape(n_new, Hkv, G, D).mean(axis=(0, 2))  # [Hkv][D]
-        big = f32_to_bf16_bits(qf / np.maximum(np.abs(qf).max(), 1e-6) * np.float32(4.0))
+        qf = bf16_bits_to_f32(q).reshape(n_new, Hkv, G, D)[n_new - 1, :, 0, :]  # [Hkv][D]: one real query row per KV head
+        big = f32_to_bf16_bits(qf / np.maximum(np.abs(qf).max(axis=-1, keepdims=True), 1e-6) * np.float32(4.0))
         if T_h > 0:
             kh[T_h - 1] = big
         kn[n_new - 1] = big

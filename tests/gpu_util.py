@@ -10,6 +10,10 @@ from paper_2606_16135_b200.runtime import Session, bits_to_torch, torch_to_bits
 
 MAX_ABS_TOL = 1e-2      # BASELINE.json north_star: bf16 output vs fp32 oracle
 REL_L2_TOL = 5e-3
+# An extra check INSIDE the stated tolerance, not a loosening: the relative L2
+# error of every single output vector (one query row of one head).  At long histories |out| ~ 0.5/sqrt(T)
+# makes the max-abs bound vacuous and a norm over a whole head could hide one corrupted row among 256.
+ROW_REL_L2_TOL = 2e-2
 
 
 def errors(out_bits: np.ndarray, ref: np.ndarray):
@@ -20,9 +24,22 @@ def errors(out_bits: np.ndarray, ref: np.ndarray):
     return max_abs, rel
 
 
+def row_errors(out_bits: np.ndarray, ref: np.ndarray) -> float:
+    """Largest relative L2 error over the output vectors (last axis = head_dim)."""
+    if not ref.size:
+        return 0.0
+    got = I.bf16_bits_to_f32(out_bits).astype(np.float64)
+    ref = ref.astype(np.float64)
+    num = np.linalg.norm(got - ref, axis=-1)
+    den = np.maximum(np.linalg.norm(ref, axis=-1), 1e-30)
+    return float((num / den).max())
+
+
 def assert_close(out_bits, ref, what=""):
     max_abs, rel = errors(out_bits, ref)
     assert max_abs <= MAX_ABS_TOL and rel <= REL_L2_TOL, f"{what}: max_abs={max_abs:.3e} rel_l2={rel:.3e}"
+    row = row_errors(out_bits, ref)
+    assert row <= ROW_REL_L2_TOL, f"{what}: worst single row rel_l2={row:.3e}"
     return max_abs, rel
 
 
@@ -30,13 +47,14 @@ class Case:
     """One conversation in one pool, mirrored in the oracle's pool."""
 
     def __init__(self, L, Hq, Hkv, D, T_h, n, NB, seed, variant="normal", identity=False, perm_id=1,
-                 lsc_extra=2, split_tiles=0, max_new=None, engine=sc.SC_ENGINE_AUTO):
+                 lsc_extra=2, split_tiles=0, max_new=None, engine=sc.SC_ENGINE_AUTO, zero_fill=True, fill_byte=None):
         self.L, self.Hq, self.Hkv, self.D, self.T_h, self.n = L, Hq, Hkv, D, T_h, n
         B = 16
         nb_total = O.blocks_for(T_h + n, B)
         assert NB >= nb_total
         self.table = I.block_table(perm_id, NB, nb_total, identity=identity)
-        self.sess = Session(L, Hq, Hkv, D, B, NB, nb_total + lsc_extra, max_new or max(n, 1))
+        self.sess = Session(L, Hq, Hkv, D, B, NB, nb_total + lsc_extra, max_new or max(n, 1),
+                            zero_fill=zero_fill, fill_byte=fill_byte)
         self.sess.pool.set_engine(engine, sc.SC_COPY_AUTO)
         if split_tiles:
             self.sess.pool.set_split_tiles(split_tiles)

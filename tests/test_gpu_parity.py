@@ -214,8 +214,31 @@ def test_resident_leading_blocks_are_read_in_place(resident):
         k, v = c.sess.read_tokens(l, 0, c.table_dev, 0, T_h + n)                 # I2 still holds
         assert np.array_equal(torch_to_bits(k), np.concatenate([c.data[l][1], c.data[l][3]]))
         assert np.array_equal(torch_to_bits(v), np.concatenate([c.data[l][2], c.data[l][4]]))
+    before = c.sess.pool.launch_count()
     with pytest.raises(sc.SwiftCacheError) as e:                                 # mma.sync engine: not supported
         c.sess.pool.set_engine(sc.SC_ENGINE_MMA_SYNC, sc.SC_COPY_AUTO)
-        c.run_layer(0, sc.SC_ATTN_STAGED)
+        c.run_layer(0, sc.SC_ATTN_STAGED, load=False)
     assert e.value.status == sc.SC_ERR_UNSUPPORTED
+    assert c.sess.pool.launch_count() == before                                  # refused before anything was launched
     c.close()
+
+
+# ------------------------------------------------------------------ memory that was never cleared
+@pytest.mark.parametrize("engine", [sc.SC_ENGINE_TCGEN05, sc.SC_ENGINE_MMA_SYNC])
+@pytest.mark.parametrize("T_h,n,split_tiles", [(333, 70, 0), (1000, 255, 2), (2049, 257, 8), (5, 3, 0)])
+def test_pool_and_lsc_prefilled_with_nan(engine, T_h, n, split_tiles):
+    """sc_pool_create(zero_fill = 0) over memory full of bf16 NaNs (0x7FC0 is not expressible as one
+    byte, 0xFF 0xFF = a NaN with every bit set): slots the conversation never wrote -- the tail of the
+    last block, unused blocks, stale LSC cells -- are masked in S, but P = 0 times a NaN V would still
+    poison the row.  The scatter zero-fills the rest of the last block, so the output must be finite
+    and within tolerance in both modes, with one CTA per pair, clusters and plain split-KV."""
+    for mode in (sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED):
+        c = Case(L=1, Hq=4, Hkv=2, D=128, T_h=T_h, n=n, NB=200, seed=991 + T_h, engine=engine,
+                 split_tiles=split_tiles, zero_fill=False, fill_byte=0xFF)
+        got = c.run_layer(0, mode)
+        assert not np.isnan(I.bf16_bits_to_f32(got)).any(), f"NaN in the output, mode {mode}"
+        assert_close(got, c.oracle_layer(0), f"nan-filled pool, engine {engine} mode {mode} T_h {T_h} n {n}")
+        k, v = c.sess.read_tokens(0, 0, c.table_dev, 0, T_h + n)                 # I2: the written tokens, bit-exact
+        assert np.array_equal(torch_to_bits(k), np.concatenate([c.data[0][1], c.data[0][3]]))
+        assert np.array_equal(torch_to_bits(v), np.concatenate([c.data[0][2], c.data[0][4]]))
+        c.close()

@@ -220,6 +220,34 @@ def test_I4_softmax_rows_sum_to_one_and_V_ones():
         assert p.shape == (T_h + n,) and abs(float(p.sum()) - 1) <= 1e-5 and (p >= 0).all()
 
 
+def test_I4_softmax_row_against_a_python_loop():
+    """sco_softmax_row_f32 against an independent pure-Python fp64 loop, e[j] / z written out:
+    a wrong scale, a wrong kv-head mapping g = h // (Hq / Hkv), a missing max subtraction that
+    overflows, or a wrong causal length T_h + i + 1 all fail here.  Config 1 (MHA) and a GQA case."""
+    for (T_h, n, Hq, Hkv, D, variant) in ((512, 32, 4, 4, 64, "normal"), (70, 9, 8, 2, 32, "peaked")):
+        q, kh, vh, kn, vn = I.make_qkv(n, T_h, Hq, Hkv, D, 77, variant)
+        K = np.concatenate([kh, kn])
+        qf = I.bf16_bits_to_f32(q).astype(np.float64)
+        Kf = I.bf16_bits_to_f32(K).astype(np.float64)
+        G = Hq // Hkv
+        for i, h in ((0, 0), (n // 2, Hq - 1), (n - 1, 1), (n - 1, Hq - 1)):
+            nk = T_h + i + 1
+            s = []
+            for j in range(nk):
+                acc = 0.0
+                for d in range(D):
+                    acc += float(qf[i, h, d]) * float(Kf[j, h // G, d])
+                s.append(acc / math.sqrt(D))
+            mx = max(s)
+            e = [math.exp(x - mx) for x in s]
+            z = sum(e)
+            want = np.array([x / z for x in e])
+            p = O.softmax_row(q, K, T_h, i, h)
+            assert p.shape == (nk,)
+            assert np.abs(p.astype(np.float64) - want).max() <= 1e-6, (T_h, i, h)
+    # the unscaled scores of the peaked case reach ~ +-60: without the max subtraction exp() overflows fp32
+
+
 def test_I4_uniform_closed_form():
     """q == 0 (or K constant) -> p uniform -> out[i] = mean(V[0 : T_h+i+1]) exactly."""
     T_h, n, Hq, Hkv, D = 45, 9, 4, 2, 16
