@@ -9,7 +9,9 @@ tokens over history + themselves, split-KV combine; two streams, double-buffered
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload lwm_5k] [--mode staged|fused]
     python bench.py --impl reference ...     # the CPU oracle, as it stands, on the host cores
 
-Prints ONE JSON line (rank 0).  See DESIGN.md section 7 for what every key means.
+Prints ONE JSON line (rank 0).  The headline is BASELINE.json configs[1] (`lwm_5k`); the other
+full-size configs are measured in the same run under `sweep` (fewer steps each).
+section 7 for what every key means.
 """
 from __future__ import annotations
 
@@ -29,6 +31,7 @@ import numpy as np  # noqa: E402
 
 METRIC = "per-turn layer-streamed prefill ms (256 new tok) & paged-KV GB/s vs HBM peak"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+SWEEP = ("lwm_50k", "gqa_128k", "gqa_128k_host", "multiturn")
 
 
 def parse_args():
@@ -43,6 +46,8 @@ def parse_args():
     ap.add_argument("--copy", default="auto", choices=["auto", "ldg", "bulk"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="only the headline workload")
+    ap.add_argument("--sweep", default=",".join(SWEEP), help="comma-separated workloads measured beside the headline")
     return ap.parse_args()
 
 
@@ -110,10 +115,25 @@ def flops_per_layer(shape, hist, n):
     return 4.0 * shape.Hq * shape.D * n * (hist + (n + 1) / 2.0)
 
 
+def config_dict(name: str, shape, mode: str, replicas: int) -> dict:
+    """`config` of the JSON line; identical in the product arm and the reference arm."""
+    kv_turn_bytes = float(sum(shape.hist)) * shape.tok_bytes * shape.L
+    return {"workload": workload_string(name, shape), "mode": mode, "replicas": replicas,
+            "l2": f"inputs larger than L2: each turn streams {kv_turn_bytes/1e9:.2f} GB of pool KV"}
+
+
+def workload_string(name: str, shape, n_new=None) -> str:
+    """Names the workload; the same string in the product arm and the reference arm."""
+    hist = list(shape.hist)
+    return (f"{name}: {shape.L} layers, {shape.Hq}q/{shape.Hkv}kv heads, D {shape.D}, block {shape.B}, "
+            f"history {hist} tokens in a shuffled {shape.n_blocks}-block "
+            f"{'pinned-host' if shape.pool_kind == 'host' else 'HBM'} pool, {n_new or shape.n_new} new tokens")
+
+
 class Workload:
     """Synthetic conversations of one BASELINE.json config, resident in HBM."""
 
-    def __init__(self, name: str, device, engine="auto", copy="auto", keep_host_layers=1):
+    def __init__(self, name: str, device, engine="auto", copy="auto", keep_host_layers=1, n_new=None):
         import torch
         from paper_2606_16135_b200 import binding as sc
         from paper_2606_16135_b200 import inputs as I
@@ -125,7 +145,7 @@ class Workload:
         B = shape.B
         self.n_seq = len(shape.hist)
         self.hist = list(shape.hist)
-        self.n_new = [shape.n_new] * self.n_seq
+        self.n_new = [n_new or shape.n_new] * self.n_seq
         self.cu = np.concatenate([[0], np.cumsum(self.n_new)]).astype(np.int32)
         blocks = [-(-(h + n * shape.turns) // B) for h, n in zip(self.hist, self.n_new)]   # room for every turn
         self.max_blocks = max(blocks)
@@ -152,7 +172,7 @@ class Workload:
                 k = I.normal_bf16_device((self.hist[s], shape.Hkv, shape.D), I.seed_for(shape.config_id, l, "k", conv=s), dev)
                 v = I.normal_bf16_device((self.hist[s], shape.Hkv, shape.D), I.seed_for(shape.config_id, l, "v", conv=s), dev)
                 self.sess.store_prefix(l, k, v, 0, self.tables_dev[s])
-                if l < keep_host_layers:
+                if l < keep_host_layers and s == 0:
                     self.host_hist[(l, s)] = (k.view(torch.int16).cpu().numpy().view(np.uint16),
                                               v.view(torch.int16).cpu().numpy().view(np.uint16))
             torch.cuda.synchronize()
@@ -212,55 +232,115 @@ class Workload:
 
 
 # ------------------------------------------------------------------ CPU baseline
-def oracle_sample(w: "Workload", rows=32, budget_s=12.0, max_steps=None):
-    """Times the CPU oracle, as it stands, on a bounded sample of the same workload: layer 0
-    of conversation 0, the whole layer's paged gather + scatter and the attention of `rows`
-    middle new-token rows over the full history, repeated until `budget_s` is spent.
-    Returns (ms per turn extrapolated to L layers x n rows x all conversations, info)."""
+class HostSample:
+    """Host (numpy) inputs of layer 0, conversation 0 of a workload for the oracle: history K/V,
+    the turn's q / k_new / v_new as bf16 bits, and a block table.  Built either from a resident
+    product workload (same bytes: the parity spot check) or, for the reference arm, from the
+    seeded host generators alone -- nothing of the product library, no GPU."""
+
+    def __init__(self, shape, kh, vh, q, kn, vn, table, hist_all, n_new_all):
+        self.shape, self.kh, self.vh, self.q, self.kn, self.vn, self.table = shape, kh, vh, q, kn, vn, table
+        self.hist_all, self.n_new_all = list(hist_all), list(n_new_all)
+
+    @classmethod
+    def from_workload(cls, w: "Workload"):
+        torch = w.torch
+        n = w.n_new[0]
+        kh, vh = w.host_hist[(0, 0)]
+        bits = lambda t: t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)   # noqa: E731
+        return cls(w.shape, kh, vh, bits(w.q[0, :n]), bits(w.k[0, :n]), bits(w.v[0, :n]),
+                   w.tables[0][:w.n_table[0]].copy(), w.hist, w.n_new)
+
+    @classmethod
+    def from_seeds(cls, name: str):
+        from paper_2606_16135_b200 import inputs as I            # seeded generators only: no method arithmetic
+        shape = I.configs()[name]
+        T_h, n = shape.hist[0], shape.n_new
+        cid = shape.config_id
+        kh = I.normal_bf16((T_h, shape.Hkv, shape.D), I.seed_for(cid, 0, "k"))
+        vh = I.normal_bf16((T_h, shape.Hkv, shape.D), I.seed_for(cid, 0, "v"))
+        q = I.normal_bf16((n, shape.Hq, shape.D), I.seed_for(cid, 0, "q"))
+        kn = I.normal_bf16((n, shape.Hkv, shape.D), I.seed_for(cid, 0, "k_new"))
+        vn = I.normal_bf16((n, shape.Hkv, shape.D), I.seed_for(cid, 0, "v_new"))
+        table = I.block_table(cid, shape.n_blocks, -(-(T_h + n) // shape.B))
+        return cls(shape, kh, vh, q, kn, vn, table, shape.hist, [n] * len(shape.hist))
+
+
+def set_omp_threads(n: int) -> bool:
+    """Thread count of the oracle's OpenMP runtime (the oracle itself is not touched)."""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
+
+
+def oracle_sample(hs: HostSample, step_budget_s=1.2, total_budget_s=12.0, max_steps=None, rows=None):
+    """Times the CPU oracle, as it stands, on a bounded sample of the workload: layer 0 of
+    conversation 0 -- the whole layer's paged gather + scatter and the attention of `rows`
+    middle new-token rows x all heads over the full history (ALL rows when they fit the step
+    budget, as at lwm_5k), repeated.  Returns (ms per turn extrapolated to L layers x n rows x
+    all conversations, info, (a, b, out))."""
     from oracle import sc_oracle as O
-    I, shape = w.I, w.shape
-    n, T_h = w.n_new[0], w.hist[0]
-    kh, vh = w.host_hist[(0, 0)]
-    tab = w.tables[0][:w.n_table[0]]
-    # the oracle's own pool, one layer deep, same block ids
-    opool = O.Pool(1, shape.Hkv, shape.D, shape.B, shape.n_blocks)
-    opool.store(0, 0, kh, 0, tab)
-    opool.store(0, 1, vh, 0, tab)
-    torch = w.torch
-    q = w.q[0, :n].view(torch.int16).cpu().numpy().view(np.uint16)
-    kn = w.k[0, :n].view(torch.int16).cpu().numpy().view(np.uint16)
-    vn = w.v[0, :n].view(torch.int16).cpu().numpy().view(np.uint16)
+    shape = hs.shape
+    n, T_h = len(hs.q), len(hs.kh)
+    tab = hs.table
+    if rows is None:      # ~2e10 flop/s is what the fp32 oracle reaches on 16 cores; never tuned, only sized
+        rows = int(max(8, min(n, step_budget_s * 2.0e10 / (4.0 * shape.Hq * shape.D * (T_h + n / 2.0)))))
+    rows = max(1, min(rows, n))
     a = max(0, n // 2 - rows // 2)
     b = min(n, a + rows)
+    # the oracle's own pool, one layer deep, same block ids
+    opool = O.Pool(1, shape.Hkv, shape.D, shape.B, shape.n_blocks)
+    opool.store(0, 0, hs.kh, 0, tab)
+    opool.store(0, 1, hs.vh, 0, tab)
     t_move, t_attn, steps, out = [], [], 0, None
     t_start = time.perf_counter()
     while True:
         t0 = time.perf_counter()
         lk = opool.gather(0, 0, tab, T_h)
         lv = opool.gather(0, 1, tab, T_h)
-        opool.store(0, 0, kn, T_h, tab)
-        opool.store(0, 1, vn, T_h, tab)
+        opool.store(0, 0, hs.kn, T_h, tab)
+        opool.store(0, 1, hs.vn, T_h, tab)
         t1 = time.perf_counter()
-        K = np.concatenate([lk, kn[:b]])
-        V = np.concatenate([lv, vn[:b]])
-        out = O.attention(q[a:b], K, V, T_h + a)
+        K = np.concatenate([lk, hs.kn[:b]])
+        V = np.concatenate([lv, hs.vn[:b]])
+        out = O.attention(hs.q[a:b], K, V, T_h + a)
         t2 = time.perf_counter()
         t_move.append(t1 - t0)
         t_attn.append(t2 - t1)
         steps += 1
-        if (max_steps and steps >= max_steps) or (not max_steps and time.perf_counter() - t_start > budget_s):
+        if (max_steps and steps >= max_steps) or (not max_steps and time.perf_counter() - t_start > total_budget_s):
             break
+    # rows [a, b) sit in the middle of the turn: their mean causal length is that of the whole turn
     scale_rows = n / float(b - a)
-    work_ratio = sum(flops_per_layer(shape, h, m) for h, m in zip(w.hist, w.n_new)) / flops_per_layer(shape, T_h, n)
-    move_ratio = sum(w.hist) / float(T_h)
+    work_ratio = (sum(flops_per_layer(shape, h, m) for h, m in zip(hs.hist_all, hs.n_new_all)) /
+                  flops_per_layer(shape, T_h, n))
+    move_ratio = sum(hs.hist_all) / float(max(T_h, 1))
     per_layer_s = np.mean(t_move) * move_ratio + np.mean(t_attn) * scale_rows * work_ratio
+    full = (b - a) == n
     info = {"cores": O.openmp_threads(), "kind": "oracle",
             "sample": (f"layer 0, conversation 0: full-layer paged gather+scatter ({np.mean(t_move)*1e3:.0f} ms) + "
-                       f"attention of new-token rows [{a},{b}) x {shape.Hq} heads over {T_h}+{n} keys "
-                       f"({np.mean(t_attn)*1e3:.0f} ms), {steps} repeats; extrapolated x{scale_rows:.0f} rows "
-                       f"x{shape.L} layers" + (f" x{work_ratio:.2f} conversations" if w.n_seq > 1 else "")),
+                       f"attention of {'ALL ' if full else ''}new-token rows [{a},{b}) x {shape.Hq} heads over {T_h}+{n} keys "
+                       f"({np.mean(t_attn)*1e3:.0f} ms), {steps} repeats; extrapolated "
+                       + ("" if full else f"x{scale_rows:.1f} rows ") + f"x{shape.L} layers"
+                       + (f" x{work_ratio:.2f} conversations" if len(hs.hist_all) > 1 else "")),
             "step_s": [float(x + y) for x, y in zip(t_move, t_attn)]}
     return per_layer_s * shape.L * 1e3, info, (a, b, out)
+
+
+def single_thread_figure(hs: HostSample) -> dict:
+    """The same oracle on ONE host thread (BASELINE.md promises it), on 1/16 of the rows."""
+    from oracle import sc_oracle as O
+    n_threads = O.openmp_threads()
+    if not set_omp_threads(1):
+        return {"unavailable": "libgomp not found"}
+    try:
+        ms, info, _ = oracle_sample(hs, max_steps=1, rows=max(4, len(hs.q) // 16))
+    finally:
+        set_omp_threads(n_threads)
+    return {"value": round(ms, 1), "unit": "ms", "cores": 1, "sample": info["sample"]}
 
 
 # ------------------------------------------------------------------ N > 1: replicas only
@@ -290,6 +370,58 @@ def whole_job(ms_per_step: float, world: int, per_replica_kv_bytes: float, per_r
 
 
 # ------------------------------------------------------------------------- ours
+def _avg(rec):
+    return rec[0] / rec[1] if rec[1] else None
+
+
+def kernel_table(w: "Workload", prof: dict, p_steps: int, staged: bool, pk: dict) -> dict:
+    """Per-kernel device time (events around every launch, inside the pipeline) against the
+    algorithmic work of DESIGN.md section 6 and the measured peaks."""
+    work = {"gather": ("hbm", w.layer_gather_bytes()), "attention": ("tensor", w.layer_flops()),
+            "scatter": ("hbm", w.layer_scatter_bytes(staged)), "combine": ("hbm", None)}
+    link = "pcie" if w.shape.pool_kind == "host" else "hbm"
+    kernels = {}
+    tot = sum(rec[0] for rec in prof.values())
+    for name, rec in prof.items():
+        a = _avg(rec)
+        if a is None:
+            continue
+        bound, amount = work[name]
+        k = {"avg_ms": round(a, 5), "launches_per_turn": rec[1] // p_steps, "share": round(rec[0] / tot, 4) if tot else None,
+             "bound": link if name == "gather" else bound}
+        if amount:
+            if bound == "hbm":
+                k["achieved_GBs"] = round(amount / a / 1e6, 1)
+                if name == "gather" and link == "pcie":
+                    k["pool_read_GBs"] = round(amount / 2 / a / 1e6, 2)          # what crosses the link: the reads
+                else:
+                    k["frac_of_measured_hbm"] = round(amount / a / 1e6 / pk["hbm_gbs"], 4)
+            else:
+                k["achieved_TFLOPs"] = round(amount / a / 1e9, 1)
+                k["frac_of_bf16_burst"] = round(amount / a / 1e9 / pk["bf16_tflops"], 4)
+                k["frac_of_bf16_sustained"] = round(amount / a / 1e9 / pk["bf16_tflops_sustained"], 4)
+        kernels[name] = k
+    return kernels
+
+
+def pinned_h2d_rate(torch, device, mb=1024) -> float:
+    """GB/s of a plain pinned cudaMemcpy host -> device, measured in this run: the link rate the
+    host-pool gather is held against."""
+    h = torch.empty(mb << 20, dtype=torch.uint8).pin_memory()
+    d = torch.empty(mb << 20, dtype=torch.uint8, device=device)
+    d.copy_(h, non_blocking=True)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best = 0.0
+    for _ in range(3):
+        e0.record()
+        d.copy_(h, non_blocking=True)
+        e1.record()
+        torch.cuda.synchronize()
+        best = max(best, (mb << 20) / e0.elapsed_time(e1) / 1e6)
+    return best
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -308,10 +440,6 @@ def run_ours(args):
     device = torch.device(f"cuda:{local}")
     torch.cuda.set_device(device)
     from paper_2606_16135_b200 import binding as sc
-
-    w = Workload(args.workload, device, args.engine, args.copy)
-    shape, pool, xs = w.shape, w.sess.pool, w.sess.compute_stream
-    mode = sc.SC_ATTN_STAGED if args.mode == "staged" else sc.SC_ATTN_FUSED
     pk = peaks()
 
     def barrier():
@@ -320,7 +448,8 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    def timed(n_steps, io="device", bufs=None):
+    def timed(w, mode, n_steps, io="device", bufs=None):
+        xs = w.sess.compute_stream
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         ev0.record(xs)
@@ -330,26 +459,39 @@ def run_ours(args):
         barrier()
         return max_over_ranks(ev0.elapsed_time(ev1), world, device)
 
+    def profile(w, mode, p_steps):
+        pool = w.sess.pool
+        pool.profile_enable(True)
+        for _ in range(p_steps):
+            w.turn(mode)
+        torch.cuda.synchronize()
+        prof = pool.profile_collect()
+        pool.profile_enable(False)
+        return prof
+
+    STAGED, FUSED = sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED
+    w = Workload(args.workload, device, args.engine, args.copy)
+    shape, pool, xs = w.shape, w.sess.pool, w.sess.compute_stream
+    mode = STAGED if args.mode == "staged" else FUSED
+
     # warm-up, then the timed region (inputs resident in HBM)
     for _ in range(max(args.warmup, 3)):
         w.turn(mode)
     barrier()
     clk = ClockSampler(local) if rank == 0 else None
     l0 = pool.launch_count()
-    total_ms = timed(args.steps)
+    total_ms = timed(w, mode, args.steps)
     launches = pool.launch_count() - l0
     clocks = clk.stop() if clk else None
     ms_per_step = total_ms / args.steps
 
     # the other variant of the path beside it (same workload, same timing protocol, fewer steps):
     # fused = attention reads pool blocks through the block table, no gather into the LSC
-    other_mode = sc.SC_ATTN_FUSED if mode == sc.SC_ATTN_STAGED else sc.SC_ATTN_STAGED
-    saved_mode, mode = mode, other_mode
+    other_mode = FUSED if mode == STAGED else STAGED
     for _ in range(3):
-        w.turn(mode)
+        w.turn(other_mode)
     o_steps = max(3, min(args.steps, 50))
-    other_ms = timed(o_steps) / o_steps
-    mode = saved_mode
+    other_ms = timed(w, other_mode, o_steps) / o_steps
 
     # end to end through the C ABI with HOST buffers (pinned): H2D of q/k/v and D2H of out inside
     e2e = None
@@ -360,20 +502,15 @@ def run_ours(args):
         for _ in range(3):
             w.turn(mode, "host", bufs)
         e_steps = max(3, min(args.steps, 20))
-        e_ms = timed(e_steps, "host", bufs) / e_steps
+        e_ms = timed(w, mode, e_steps, "host", bufs) / e_steps
         h2d = sum(int(t.numel()) * 2 for t in (hq, hk, hv))
         d2h = int(hout.numel()) * 2
         e2e = {"value": round(e_ms, 4), "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "pcie_gbs": round((h2d + d2h) / e_ms / 1e6, 2)}
 
     # per-kernel device times: events around every launch, on its own stream, inside the pipeline
-    pool.profile_enable(True)
     p_steps = 5
-    for _ in range(p_steps):
-        w.turn(mode)
-    torch.cuda.synchronize()
-    prof = pool.profile_collect()
-    pool.profile_enable(False)
+    prof = profile(w, mode, p_steps)
     # and each kernel alone (no concurrent stream): gather over all layers, fused attention
     iso = {}
     st = xs.cuda_stream
@@ -388,65 +525,56 @@ def run_ours(args):
         for l in range(shape.L):
             pool.prefill_layer_batched(l, w.q[l].data_ptr(), w.k[l].data_ptr(), w.v[l].data_ptr(),
                                        w.tables_dev.data_ptr(), w.max_blocks, w.hist, w.cu, 0,
-                                       sc.SC_ATTN_FUSED, w.out[l].data_ptr(), st)
+                                       FUSED, w.out[l].data_ptr(), st)
     torch.cuda.synchronize()
     c = pool.profile_collect()
     iso["attention_fused"], iso["scatter"], iso["combine"] = c["attention"], c["scatter"], c["combine"]
     pool.profile_enable(False)
 
-    def avg(rec):
-        return rec[0] / rec[1] if rec[1] else None
-
-    staged = mode == sc.SC_ATTN_STAGED
+    staged = mode == STAGED
+    kernels = kernel_table(w, prof, p_steps, staged, pk)
     work = {"gather": ("hbm", w.layer_gather_bytes()), "attention": ("tensor", w.layer_flops()),
-            "scatter": ("hbm", w.layer_scatter_bytes(staged)), "combine": ("hbm", None)}
-    kernels = {}
-    for name, rec in prof.items():
-        a = avg(rec)
-        if a is None:
-            continue
-        bound, amount = work[name]
-        k = {"avg_ms": round(a, 5), "launches_per_turn": rec[1] // p_steps, "share": None, "bound": bound}
-        if amount:
-            if bound == "hbm":
-                k["achieved_GBs"] = round(amount / a / 1e6, 1)
-                k["frac_of_measured_hbm"] = round(amount / a / 1e6 / pk["hbm_gbs"], 4)
-            else:
-                k["achieved_TFLOPs"] = round(amount / a / 1e9, 1)
-                k["frac_of_measured_bf16_sustained"] = round(amount / a / 1e9 / pk["bf16_tflops_sustained"], 4)
-        kernels[name] = k
-    tot = sum(rec[0] for rec in prof.values())
-    for name, rec in prof.items():
-        if name in kernels:
-            kernels[name]["share"] = round(rec[0] / tot, 4)
-    dom = max((n for n in prof if work[n][1]), key=lambda n: prof[n][0])
-    d_avg = avg(prof[dom])
+            "scatter": ("hbm", w.layer_scatter_bytes(staged))}
+    dom = max((n for n in prof if n in work and prof[n][1]), key=lambda n: prof[n][0])
+    d_avg = _avg(prof[dom])
     bound, amount = work[dom]
-    traffic = None
+    traffic, traffic_src = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic.txt")
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get(f"{args.workload}:{dom}")
+            tj = json.load(f)
+        traffic = tj.get(f"{args.workload}:{args.mode}:{dom}")
+        traffic_src = tj.get("_source") if traffic is not None else None
     if bound == "hbm":
         roof = {"kernel": dom, "bound": "hbm", "achieved": round(amount / d_avg / 1e6, 1), "peak": pk["hbm_gbs"],
                 "unit": "GB/s", "peak_source": pk["_source"] + " copy bandwidth"}
     else:
+        # burst peak: the timed region is milliseconds long at the maximum SM clock (see `clocks`), not the
+        # seconds-long power-capped regime the sustained figure describes; the sustained fraction is beside it
         roof = {"kernel": dom, "bound": "tensor", "achieved": round(amount / d_avg / 1e9, 1),
-                "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
-                "peak_source": pk["_source"] + " cuBLAS bf16, sustained (kernel timed inside a long step)"}
+                "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
+                "peak_source": pk["_source"] + " cuBLAS bf16, burst",
+                "frac_of_sustained_peak": round(amount / d_avg / 1e9 / pk["bf16_tflops_sustained"], 4)}
     roof["frac"] = round(roof["achieved"] / roof["peak"], 4)
     roof["traffic"] = traffic
+    roof["traffic_source"] = traffic_src       # a committed ncu capture of an earlier run of this command, not this run
     roof["avg_launch_ms"] = round(d_avg, 5)
+    roof["timed"] = "inside the two-stream pipeline" if staged else "fused turn, one stream"
+    af = _avg(iso["attention_fused"])
+    if af:
+        roof["attention_alone"] = {"avg_launch_ms": round(af, 5), "achieved": round(w.layer_flops() / af / 1e9, 1),
+                                   "frac": round(w.layer_flops() / af / 1e9 / pk["bf16_tflops"], 4)}
 
     # the oracle beside it (rank 0, bounded sample) and a parity spot check on that sample
     cpu, parity = None, None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu_ms, info, (a, b, ref) = oracle_sample(w)
+        hs = HostSample.from_workload(w)
+        cpu_ms, info, (a, b, ref) = oracle_sample(hs)
         got = w.I.bf16_bits_to_f32(w.out[0, a:b].view(torch.int16).cpu().numpy().view(np.uint16)).astype(np.float64)
         parity = {"layer": 0, "rows": [a, b], "max_abs": float(np.abs(got - ref).max()),
                   "rel_l2": float(np.linalg.norm(got - ref) / np.linalg.norm(ref)), "tol": [1e-2, 5e-3]}
         info.pop("step_s")
-        cpu = {"value": round(cpu_ms, 1), "unit": "ms", **info}
+        cpu = {"value": round(cpu_ms, 1), "unit": "ms", **info, "single_thread": single_thread_figure(hs)}
 
     kv_turn_bytes = w.layer_hist_kv_bytes() * shape.L
     job = whole_job(ms_per_step, world, kv_turn_bytes, w.layer_flops() * shape.L)
@@ -454,66 +582,121 @@ def run_ours(args):
         "metric": METRIC, "value": round(ms_per_step, 4), "unit": "ms", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: {shape.L} layers, {shape.Hq}q/{shape.Hkv}kv heads, D {shape.D}, "
-                               f"block {shape.B}, history {list(w.hist)} tokens in a shuffled {shape.n_blocks}-block "
-                               f"{'pinned-host' if shape.pool_kind == 'host' else 'HBM'} pool, {shape.n_new} new tokens",
-                   "mode": args.mode, "replicas": world,
-                   "l2": f"inputs larger than L2: each turn streams {kv_turn_bytes/1e9:.2f} GB of pool KV"},
+        "config": config_dict(args.workload, shape, args.mode, world),
         "kv_gbs": round(job["kv_gbs"], 1),
         "attn_tflops": round(job["attn_tflops"], 1),
-        "other_mode": {"mode": "fused" if other_mode == sc.SC_ATTN_FUSED else "staged", "value": round(other_ms, 4),
+        "other_mode": {"mode": "fused" if other_mode == FUSED else "staged", "value": round(other_ms, 4),
                        "unit": "ms", "steps": o_steps},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof, "kernels": kernels,
-        "isolated": {k: {"avg_ms": round(avg(v), 5)} for k, v in iso.items() if avg(v) is not None},
+        "isolated": {k: {"avg_ms": round(_avg(v), 5)} for k, v in iso.items() if _avg(v) is not None},
         "cpu_baseline": cpu, "parity": parity,
     }
-    g = avg(iso["gather"])
+    g = _avg(iso["gather"])
     if g:
         line["isolated"]["gather"]["GBs"] = round(w.layer_gather_bytes() / g / 1e6, 1)
         line["isolated"]["gather"]["frac_of_measured_hbm"] = round(w.layer_gather_bytes() / g / 1e6 / pk["hbm_gbs"], 4)
-    af = avg(iso["attention_fused"])
     if af:
         line["isolated"]["attention_fused"]["TFLOPs"] = round(w.layer_flops() / af / 1e9, 1)
         line["isolated"]["attention_fused"]["kv_read_GBs"] = round(w.layer_hist_kv_bytes() / af / 1e6, 1)
+    w.sess.close()
+    del w
+    torch.cuda.empty_cache()
+
+    # ---- the other full-size configs of BASELINE.json, same protocol, fewer steps (rank 0 of a 1-GPU run) ----
+    if rank == 0 and world == 1 and not args.no_sweep and args.workload == "lwm_5k":
+        line["sweep"] = run_sweep(args, device, timed, profile, pk, local)
     if rank == 0:
         print(json.dumps(line))
-    w.sess.close()
     if world > 1:
         dist.destroy_process_group()
 
 
+def run_sweep(args, device, timed, profile, pk, local) -> dict:
+    """lwm_50k, gqa_128k (HBM and pinned-host pool), multiturn (turns 0 and 9): ms per turn in both
+    modes, per-kernel averages against the measured peaks, clocks sampled during each timed region."""
+    import torch
+    from paper_2606_16135_b200 import binding as sc
+    STAGED, FUSED = sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED
+    out = {}
+    h2d_rate = None
+    for name in [x for x in args.sweep.split(",") if x]:
+        t_begin = time.perf_counter()
+        try:
+            w = Workload(name, device, args.engine, args.copy, keep_host_layers=0)
+        except Exception as e:                    # e.g. not enough pinned host memory on this box
+            out[name] = {"unavailable": f"{type(e).__name__}: {e}"[:200]}
+            continue
+        shape = w.shape
+        host = shape.pool_kind == "host"
+        steps = 3 if host else (5 if name != "lwm_50k" else 10)
+        entry = {"workload": workload_string(name, shape), "steps": steps, "warmup": 3}
+
+        def measure(dst):
+            for m, mname in ((STAGED, "staged"), (FUSED, "fused")):
+                for _ in range(3):
+                    w.turn(m)
+                clk = ClockSampler(local)
+                ms = timed(w, m, steps) / steps
+                c = clk.stop()
+                prof = profile(w, m, 2)
+                dst[mname] = {"ms_per_turn": round(ms, 3),
+                              "kv_gbs": round(w.layer_hist_kv_bytes() * shape.L / ms / 1e6, 1),
+                              "attn_tflops": round(w.layer_flops() * shape.L / ms / 1e9, 1),
+                              "kernels": kernel_table(w, prof, 2, m == STAGED, pk),
+                              "clocks": {k: c[k] for k in ("sm_mhz", "sm_max_mhz", "reasons")}}
+
+        measure(entry)
+        if host:
+            h2d_rate = h2d_rate or pinned_h2d_rate(torch, device)
+            g = entry["staged"]["kernels"].get("gather", {})
+            entry["pcie"] = {"pinned_memcpy_h2d_GBs": round(h2d_rate, 2), "gather_pool_read_GBs": g.get("pool_read_GBs"),
+                             "frac_of_memcpy_rate": round(g["pool_read_GBs"] / h2d_rate, 4) if g.get("pool_read_GBs") else None}
+        if shape.turns > 1:                         # config 5: ten successive turns; turn 0 above, now the last one
+            entry["turn"] = 0
+            for t in range(1, shape.turns):
+                w.turn(FUSED)                       # the turn's new KV becomes history (scattered into the pool)
+                w.advance(t)
+            last = {"turn": shape.turns - 1, "history": list(w.hist)}
+            measure(last)
+            entry[f"turn_{shape.turns - 1}"] = last
+        entry["wall_s"] = round(time.perf_counter() - t_begin, 1)
+        out[name] = entry
+        w.sess.close()
+        del w
+        torch.cuda.empty_cache()
+    return out
+
+
 # -------------------------------------------------------------------- reference
 def run_reference(args):
-    """The CPU oracle, as it stands, on the host cores: same config, metric and unit.  Each
-    step is a bounded sample of the workload (see oracle_sample); rank 0 only."""
+    """The CPU oracle, as it stands, on the host cores: same config, metric and unit.  Touches
+    nothing of the product library and no GPU: inputs come from the seeded host generators
+    (paper_2606_16135_b200/inputs.py holds no method arithmetic), the table from inputs.block_table.
+    Each step is a bounded sample of the workload (see oracle_sample) sized so that
+    --steps K --warmup W ends within a few minutes; rank 0 only."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import torch
-    if not torch.cuda.is_available():
-        print(json.dumps({"impl": "reference", "unavailable": "inputs are generated on the CUDA device"}))
-        return
-    from paper_2606_16135_b200 import build as sc_build
-    sc_build.build()
-    w = Workload(args.workload, torch.device("cuda:0"))
-    shape = w.shape
-    oracle_sample(w, max_steps=max(args.warmup, 1))
-    ms, info, _ = oracle_sample(w, max_steps=args.steps)
+    from paper_2606_16135_b200 import inputs as I
+    shape = I.configs()[args.workload]
+    hs = HostSample.from_seeds(args.workload)
+    n_steps = max(args.steps, 1)
+    step_budget = min(1.2, 150.0 / (n_steps + max(args.warmup, 1)))
+    oracle_sample(hs, step_budget_s=step_budget, max_steps=max(args.warmup, 1))
+    ms, info, _ = oracle_sample(hs, step_budget_s=step_budget, max_steps=n_steps)
     step_s = info.pop("step_s")
+    cpu = {"value": round(ms, 1), "unit": "ms", **info, "single_thread": single_thread_figure(hs)}
     line = {
         "impl": "reference", "metric": METRIC, "value": round(ms, 1), "unit": "ms", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(float(np.mean(step_s)) * 1e3, 2),
         "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: {shape.L} layers, {shape.Hq}q/{shape.Hkv}kv heads, D {shape.D}, "
-                               f"block {shape.B}, history {list(w.hist)} tokens, {shape.n_new} new tokens",
-                   "mode": "oracle"},
-        "cpu_baseline": {"value": round(ms, 1), "unit": "ms", **info},
+        "config": config_dict(args.workload, shape, args.mode, 1),
+        "cpu_baseline": cpu,
         "e2e": {"value": round(ms, 1), "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
-    w.sess.close()
 
 
 if __name__ == "__main__":

@@ -231,6 +231,33 @@ sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_al
                             const int32_t *hist_lens, const int32_t *cu_new, int32_t mode,
                             void *copy_stream, void *compute_stream);
 
+/* a8 with options -- SURVEY.md 8(f) row f4.  The paper's own pipeline has ONE active-layer buffer
+ * and hides the load behind the model's other work: "the (i)-th layer's load is blocked until
+ * both the attention computation and KV store of the (i-1)-th layer are complete; the load then
+ * overlaps with the FFN of layer i-1" (Fig. 10 at :404).
+ *   lsc_buffers = 2 : sc_prefill_turn's schedule (reading S8): load(l+1) -> LSC[(l+1)%2] runs beside
+ *                     attention(l) and waits for attention(l-1);
+ *   lsc_buffers = 1 : the paper's: only LSC[0] is used; load(l+1) waits for attention(l) (which
+ *                     follows the scatter = "KV store" of layer l on the same stream), attention(l+1)
+ *                     waits for load(l+1).  Whatever the hook enqueues after attention(l) on the
+ *                     compute stream (the model's o-proj / FFN) is what the load can hide behind.
+ *   after_attention : may be NULL.  Called ON THE HOST, synchronously, once per layer, right after
+ *                     layer l's attention (and, in STAGED mode with one buffer, the load of layer
+ *                     l+1) has been enqueued; it may enqueue work on compute_stream and must not
+ *                     synchronise.  The library neither reads nor writes what it enqueues.
+ * opt == NULL means {2, NULL, NULL}.  Everything else as sc_prefill_turn.                       */
+typedef void (*sc_layer_hook_t)(int32_t layer, void *compute_stream, void *user);
+typedef struct {
+    int32_t lsc_buffers;             /* 1 or 2 */
+    sc_layer_hook_t after_attention; /* HOST callback, may be NULL */
+    void *user;                      /* passed through to the hook */
+} sc_turn_options_t;
+sc_status_t sc_prefill_turn_ex(sc_pool_t *pool, const void *q_all, const void *k_all,
+                               const void *v_all, void *out_all, int32_t io_kind,
+                               const int32_t *tables_dev, int32_t max_blocks, int32_t n_seq,
+                               const int32_t *hist_lens, const int32_t *cu_new, int32_t mode,
+                               void *copy_stream, void *compute_stream, const sc_turn_options_t *opt);
+
 /* Per-kernel timing for measurement (bench.py's roofline): while enabled, every kernel
  * launch is bracketed by CUDA events on the stream it is launched on.  Enabling clears
  * earlier records.  sc_profile_collect waits for the recorded events and returns, per

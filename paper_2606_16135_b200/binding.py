@@ -39,7 +39,7 @@ SYMBOLS = [
     "sc_read_tokens", "sc_load_layer", "sc_prefill_layer", "sc_load_layer_batched",
     "sc_prefill_layer_batched", "sc_prefill_turn", "sc_launch_count", "sc_profile_enable",
     "sc_profile_collect", "sc_lsc_rc_sizing", "sc_elastic_units", "sc_scale_up", "sc_scale_down",
-    "sc_pool_resize", "sc_set_resident_blocks",
+    "sc_pool_resize", "sc_set_resident_blocks", "sc_prefill_turn_ex",
 ]
 
 
@@ -59,6 +59,13 @@ class sc_pool_info_t(C.Structure):
 class sc_sizing_t(C.Structure):
     _fields_ = [("k_master", C.c_int64), ("sum_k", C.c_int64), ("n_lsc", C.c_int64), ("n_rc", C.c_int64),
                 ("max_context_blocks", C.c_int64), ("conventional_blocks", C.c_int64)]
+
+
+LAYER_HOOK = C.CFUNCTYPE(None, C.c_int32, C.c_void_p, C.c_void_p)
+
+
+class sc_turn_options_t(C.Structure):
+    _fields_ = [("lsc_buffers", C.c_int32), ("after_attention", LAYER_HOOK), ("user", C.c_void_p)]
 
 
 class SwiftCacheError(RuntimeError):
@@ -103,6 +110,8 @@ def lib() -> C.CDLL:
         "sc_load_layer_batched": [vp, i32, vp, i32, i32, i32p, i32p, i32, vp],
         "sc_prefill_layer_batched": [vp, i32, vp, vp, vp, vp, i32, i32, i32p, i32p, i32, i32, vp, vp],
         "sc_prefill_turn": [vp, vp, vp, vp, vp, i32, vp, i32, i32, i32p, i32p, i32, vp, vp],
+        "sc_prefill_turn_ex": [vp, vp, vp, vp, vp, i32, vp, i32, i32, i32p, i32p, i32, vp, vp,
+                               C.POINTER(sc_turn_options_t)],
         "sc_launch_count": [vp, C.POINTER(i64)],
         "sc_profile_enable": [vp, i32],
         "sc_profile_collect": [vp, C.POINTER(C.c_double), C.POINTER(i64)],
@@ -304,3 +313,16 @@ class Pool:
         check(lib().sc_prefill_turn(self._h, q_all_ptr, k_all_ptr, v_all_ptr, out_all_ptr, io_kind,
                                     tables_ptr, max_blocks, len(h), hp, cp, mode, copy_stream or None,
                                     compute_stream or None))
+
+    def prefill_turn_ex(self, q_all_ptr, k_all_ptr, v_all_ptr, out_all_ptr, io_kind, tables_ptr,
+                        max_blocks, hist_lens, cu_new, mode, copy_stream, compute_stream,
+                        lsc_buffers=2, after_attention=None):
+        """`after_attention(layer, compute_stream_handle)` is a Python callable run on the host
+        after each layer has been enqueued (it may enqueue work on the compute stream)."""
+        h, hp = _i32_array(hist_lens)
+        c, cp = _i32_array(cu_new)
+        hook = LAYER_HOOK(lambda layer, stream, user: after_attention(layer, stream)) if after_attention else LAYER_HOOK()
+        opt = sc_turn_options_t(lsc_buffers, hook, None)
+        check(lib().sc_prefill_turn_ex(self._h, q_all_ptr, k_all_ptr, v_all_ptr, out_all_ptr, io_kind,
+                                       tables_ptr, max_blocks, len(h), hp, cp, mode, copy_stream or None,
+                                       compute_stream or None, C.byref(opt)))

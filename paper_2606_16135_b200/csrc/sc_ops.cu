@@ -356,8 +356,20 @@ sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_al
                             int32_t max_blocks, int32_t n_seq, const int32_t *hist_lens,
                             const int32_t *cu_new, int32_t mode, void *copy_stream, void *compute_stream)
 {
+    return sc_prefill_turn_ex(pool, q_all, k_all, v_all, out_all, io_kind, tables_dev, max_blocks, n_seq, hist_lens,
+                              cu_new, mode, copy_stream, compute_stream, nullptr);
+}
+
+sc_status_t sc_prefill_turn_ex(sc_pool_t *pool, const void *q_all, const void *k_all, const void *v_all,
+                               void *out_all, int32_t io_kind, const int32_t *tables_dev,
+                               int32_t max_blocks, int32_t n_seq, const int32_t *hist_lens,
+                               const int32_t *cu_new, int32_t mode, void *copy_stream, void *compute_stream,
+                               const sc_turn_options_t *opt)
+{
     sc_status_t st = check_pool(pool, 0);
     if (st) return st;
+    const int nbuf = opt ? opt->lsc_buffers : 2;
+    if (nbuf != 1 && nbuf != 2) return sc_fail(SC_ERR_INVALID_ARG, "lsc_buffers %d not in {1,2}", nbuf);
     if (!q_all || !k_all || !v_all || !out_all) return sc_fail(SC_ERR_INVALID_ARG, "NULL tensor");
     if (io_kind != SC_MEM_DEVICE && io_kind != SC_MEM_HOST_PINNED) return sc_fail(SC_ERR_INVALID_ARG, "io_kind %d", io_kind);
     if (mode != SC_ATTN_STAGED && mode != SC_ATTN_FUSED) return sc_fail(SC_ERR_INVALID_ARG, "mode %d", mode);
@@ -397,12 +409,13 @@ sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_al
         SC_CUDA(cudaStreamWaitEvent(pool->d2h_stream, pool->ev_fork, 0));
     }
     for (int l = 0; l < L; ++l) {
-        const int bf = l & 1;
+        const int bf = (nbuf == 2) ? (l & 1) : 0;      // LSC buffer of this layer
+        const int sb2 = l & 1;                         // host-io staging slot of this layer
         const char *q = (const char *)q_all + (int64_t)l * q_bytes;
         const char *k = (const char *)k_all + (int64_t)l * kv_bytes;
         const char *v = (const char *)v_all + (int64_t)l * kv_bytes;
         char *o = (char *)out_all + (int64_t)l * q_bytes;
-        if (staged && l + 1 < L) {
+        if (staged && nbuf == 2 && l + 1 < L) {
             // load(l+1) overwrites LSC[bf^1], last read by attention(l-1)
             if (l >= 1) SC_CUDA(cudaStreamWaitEvent(cs, pool->ev_attn[bf ^ 1], 0));
             st = sc_load_layer_batched(pool, l + 1, tables_dev, max_blocks, n_seq, hist_lens, cu_new, bf ^ 1, cs);
@@ -412,14 +425,14 @@ sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_al
         const char *dq = q, *dk = k, *dv = v;
         char *dout = o;
         if (host_io) {
-            char *sb = pool->stage[bf];
-            if (l >= 2) SC_CUDA(cudaStreamWaitEvent(pool->h2d_stream, pool->ev_comp[bf], 0));
+            char *sb = pool->stage[sb2];
+            if (l >= 2) SC_CUDA(cudaStreamWaitEvent(pool->h2d_stream, pool->ev_comp[sb2], 0));
             SC_CUDA(cudaMemcpyAsync(sb, q, (size_t)q_bytes, cudaMemcpyHostToDevice, pool->h2d_stream));
             SC_CUDA(cudaMemcpyAsync(sb + q_bytes, k, (size_t)kv_bytes, cudaMemcpyHostToDevice, pool->h2d_stream));
             SC_CUDA(cudaMemcpyAsync(sb + q_bytes + kv_bytes, v, (size_t)kv_bytes, cudaMemcpyHostToDevice, pool->h2d_stream));
-            SC_CUDA(cudaEventRecord(pool->ev_h2d[bf], pool->h2d_stream));
-            SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_h2d[bf], 0));
-            if (l >= 2) SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_d2h[bf], 0));
+            SC_CUDA(cudaEventRecord(pool->ev_h2d[sb2], pool->h2d_stream));
+            SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_h2d[sb2], 0));
+            if (l >= 2) SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_d2h[sb2], 0));
             dq = sb; dk = sb + q_bytes; dv = sb + q_bytes + kv_bytes; dout = sb + q_bytes + 2 * kv_bytes;
         }
         if (staged) SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_load[bf], 0));
@@ -427,12 +440,21 @@ sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_al
                                       mode, dout, xs);
         if (st) return st;
         if (staged) SC_CUDA(cudaEventRecord(pool->ev_attn[bf], xs));
-        if (host_io) {
-            SC_CUDA(cudaEventRecord(pool->ev_comp[bf], xs));
-            SC_CUDA(cudaStreamWaitEvent(pool->d2h_stream, pool->ev_comp[bf], 0));
-            SC_CUDA(cudaMemcpyAsync(o, dout, (size_t)q_bytes, cudaMemcpyDeviceToHost, pool->d2h_stream));
-            SC_CUDA(cudaEventRecord(pool->ev_d2h[bf], pool->d2h_stream));
+        if (staged && nbuf == 1 && l + 1 < L) {
+            // the paper's ordering: load(l+1) into the ONE buffer waits for attention(l) and store(l)
+            // (PAPER.md:192); it then runs beside whatever the hook puts on the compute stream
+            SC_CUDA(cudaStreamWaitEvent(cs, pool->ev_attn[0], 0));
+            st = sc_load_layer_batched(pool, l + 1, tables_dev, max_blocks, n_seq, hist_lens, cu_new, 0, cs);
+            if (st) return st;
+            SC_CUDA(cudaEventRecord(pool->ev_load[0], cs));
         }
+        if (host_io) {
+            SC_CUDA(cudaEventRecord(pool->ev_comp[sb2], xs));
+            SC_CUDA(cudaStreamWaitEvent(pool->d2h_stream, pool->ev_comp[sb2], 0));
+            SC_CUDA(cudaMemcpyAsync(o, dout, (size_t)q_bytes, cudaMemcpyDeviceToHost, pool->d2h_stream));
+            SC_CUDA(cudaEventRecord(pool->ev_d2h[sb2], pool->d2h_stream));
+        }
+        if (opt && opt->after_attention) opt->after_attention(l, compute_stream, opt->user);
     }
     if (host_io) {   // join: the compute stream finishes last
         SC_CUDA(cudaStreamWaitEvent(xs, pool->ev_d2h[(L - 1) & 1], 0));

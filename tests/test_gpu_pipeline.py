@@ -227,6 +227,52 @@ def test_pipeline_ordering_survives_a_slow_stream(slow):
     cv.sess.close()
 
 
+@pytest.mark.parametrize("slow", [None, "copy", "compute"])
+@pytest.mark.parametrize("mode", [sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED])
+def test_single_buffer_paper_ordering(mode, slow):
+    """f4 (Fig. 10 at :404): ONE LSC buffer, load(l+1) waits for attention(l) and the
+    store of layer l, and hides behind what the model does next -- here a hook that puts a GEMM on
+    the compute stream after every attention.  Same oracle, same answer bit for bit as the
+    two-buffer schedule, also with one stream held up right before the turn."""
+    cv = Conversations(L=6, Hq=4, Hkv=4, D=128, hist=[1500, 300], NB=260, max_new=200, seed=23)
+    p, dev = cv.sess.pool, cv.sess.device
+    n_new = [100, 37]
+    cv.begin_turn(n_new)
+    q_all, k_all, v_all = cv.make_inputs(n_new, 811)
+    ref = cv.oracle_turn(q_all, k_all, v_all)
+    tq, tk, tv = (bits_to_torch(x, dev) for x in (q_all, k_all, v_all))
+    out2, out1 = torch.zeros_like(tq), torch.zeros_like(tq)
+    wa = torch.randn(512, 512, device=dev)
+    seen = []
+
+    def hook(layer, stream_handle):
+        assert stream_handle == cv.sess.compute_stream.cuda_stream
+        seen.append(layer)
+        with torch.cuda.stream(cv.sess.compute_stream):
+            torch.matmul(wa, wa)                          # the "FFN" the load hides behind
+
+    torch.cuda.synchronize()
+    args = (sc.SC_MEM_DEVICE, cv.tables_dev.data_ptr(), cv.max_blocks, cv.hist, cv.cu, mode,
+            cv.sess.copy_stream.cuda_stream, cv.sess.compute_stream.cuda_stream)
+    p.prefill_turn(tq.data_ptr(), tk.data_ptr(), tv.data_ptr(), out2.data_ptr(), *args)
+    torch.cuda.synchronize()
+    if slow:
+        with torch.cuda.stream(cv.sess.copy_stream if slow == "copy" else cv.sess.compute_stream):
+            torch.cuda._sleep(int(2e8))
+    p.prefill_turn_ex(tq.data_ptr(), tk.data_ptr(), tv.data_ptr(), out1.data_ptr(), *args,
+                      lsc_buffers=1, after_attention=hook)
+    torch.cuda.synchronize()
+    assert seen == list(range(cv.L))
+    assert torch.equal(out1.view(torch.int16), out2.view(torch.int16))
+    for l in range(cv.L):
+        assert_close(torch_to_bits(out1[l]), ref[l], f"single buffer, mode {mode}, slow {slow}: layer {l}")
+    cv.end_turn(n_new)
+    cv.check_pool_equals_logical()
+    with pytest.raises(sc.SwiftCacheError):
+        p.prefill_turn_ex(tq.data_ptr(), tk.data_ptr(), tv.data_ptr(), out1.data_ptr(), *args, lsc_buffers=3)
+    cv.sess.close()
+
+
 def test_block_major_resize_on_the_device():
     """f1 (PAPER.md:214-216): growing the pool appends blocks and releasing the tail frees them;
     no existing block moves -- the conversation's KV reads back bit-exactly through the same
