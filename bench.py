@@ -422,6 +422,91 @@ def pinned_h2d_rate(torch, device, mb=1024) -> float:
     return best
 
 
+class Filler:
+    """The work a model does between two attentions -- o-proj, FFN (gate, up, down) of layer l and the
+    QKV projection of layer l+1 for the turn's new tokens, Llama-2-7B sizes, random weights -- as ONE
+    CUDA graph of cuBLAS GEMMs.  It is NOT on the method's path (the GEMMs are
+    outside); the f4 harness only needs something of the right length on the compute stream for the
+    single-buffer load to hide behind."""
+
+    def __init__(self, torch, device, stream, n_tokens, hidden, ffn=11008):
+        self.torch, self.stream = torch, stream
+        bf = torch.bfloat16
+        self.x = torch.randn(n_tokens, hidden, device=device, dtype=bf)
+        self.wo = torch.randn(hidden, hidden, device=device, dtype=bf) * 0.01
+        self.w13 = torch.randn(hidden, 2 * ffn, device=device, dtype=bf) * 0.01
+        self.w2 = torch.randn(ffn, hidden, device=device, dtype=bf) * 0.01
+        self.wqkv = torch.randn(hidden, 3 * hidden, device=device, dtype=bf) * 0.01
+        self.ffn = ffn
+        self.flops = 2.0 * n_tokens * hidden * (hidden + 2 * ffn + ffn + 3 * hidden)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(stream):
+            self._body()                                  # warm cuBLAS up outside the capture
+        torch.cuda.synchronize()
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph, stream=stream):
+            self._body()
+        torch.cuda.synchronize()
+
+    def _body(self):
+        t = self.torch
+        h = t.matmul(self.x, self.wo)
+        g = t.matmul(h, self.w13)
+        a = g[:, :self.ffn] * g[:, self.ffn:]
+        y = t.matmul(a, self.w2)
+        self.y = t.matmul(y, self.wqkv)
+
+    def __call__(self, layer=None, stream_handle=None):
+        with self.torch.cuda.stream(self.stream):
+            self.graph.replay()
+
+
+def measure_overlap(w: "Workload", timed_fn, steps: int) -> dict:
+    """the paper's single-buffer schedule (sc_prefill_turn_ex, lsc_buffers = 1).
+    Exposed load time per layer = (turn with loads) - (the same compute with no loads), measured once
+    with nothing between the attentions (nothing to hide behind) and once with the Filler GEMMs
+    enqueued after every attention by the hook."""
+    torch, sc = w.torch, w.sc
+    pool, sess, shape = w.sess.pool, w.sess, w.shape
+    L = shape.L
+    fill = Filler(torch, sess.device, sess.compute_stream, int(w.cu[-1]), shape.Hq * shape.D)
+    # the same GEMMs over a 4096-token batch (many conversations prefilled together): compute-bound,
+    # where the turn's own tokens make them stream their weights, i.e. HBM-bound like the load itself
+    fill_big = Filler(torch, sess.device, sess.compute_stream, 4096, shape.Hq * shape.D)
+    xs = sess.compute_stream.cuda_stream
+
+    def turn_ex(nbuf, hook):
+        pool.prefill_turn_ex(w.q.data_ptr(), w.k.data_ptr(), w.v.data_ptr(), w.out.data_ptr(), sc.SC_MEM_DEVICE,
+                             w.tables_dev.data_ptr(), w.max_blocks, w.hist, w.cu, sc.SC_ATTN_STAGED,
+                             sess.copy_stream.cuda_stream, xs, lsc_buffers=nbuf, after_attention=hook)
+
+    def compute_only(hook):
+        # the same scatter + attention per layer reading LSC[0] as it stands (no load): timing reference
+        for l in range(L):
+            pool.prefill_layer_batched(l, w.q[l].data_ptr(), w.k[l].data_ptr(), w.v[l].data_ptr(),
+                                       w.tables_dev.data_ptr(), w.max_blocks, w.hist, w.cu, 0,
+                                       sc.SC_ATTN_STAGED, w.out[l].data_ptr(), xs)
+            if hook:
+                hook(l, xs)
+
+    res = {}
+    for tag, hook in (("no_filler", None), ("filler", fill), ("filler_4096_tokens", fill_big)):
+        t = {}
+        for name, fn in (("single_buffer", lambda: turn_ex(1, hook)), ("double_buffer", lambda: turn_ex(2, hook)),
+                         ("compute_only", lambda: compute_only(hook))):
+            for _ in range(2):
+                fn()
+            t[name] = timed_fn(fn, steps) / steps
+        res[tag] = {"single_buffer_ms": round(t["single_buffer"], 3), "double_buffer_ms": round(t["double_buffer"], 3),
+                    "compute_only_ms": round(t["compute_only"], 3),
+                    "exposed_load_ms_per_layer": round(max(0.0, t["single_buffer"] - t["compute_only"]) / L, 4),
+                    "exposed_load_pct_of_turn": round(100.0 * max(0.0, t["single_buffer"] - t["compute_only"]) / t["single_buffer"], 2)}
+    res["filler"]["filler_gflop_per_layer"] = round(fill.flops / 1e9, 1)
+    res["filler_4096_tokens"]["filler_gflop_per_layer"] = round(fill_big.flops / 1e9, 1)
+    res["schedule"] = "lsc_buffers=1: load(l+1) waits attention(l)+store(l), then runs beside the hook's GEMMs (PAPER.md:192)"
+    return res
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -458,6 +543,16 @@ def run_ours(args):
         ev1.record(xs)
         barrier()
         return max_over_ranks(ev0.elapsed_time(ev1), world, device)
+
+    def timed_fn(fn, n_steps, stream=None):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        ev0.record(stream)
+        for _ in range(n_steps):
+            fn()
+        ev1.record(stream)
+        barrier()
+        return ev0.elapsed_time(ev1)
 
     def profile(w, mode, p_steps):
         pool = w.sess.pool
@@ -599,20 +694,51 @@ def run_ours(args):
     if af:
         line["isolated"]["attention_fused"]["TFLOPs"] = round(w.layer_flops() / af / 1e9, 1)
         line["isolated"]["attention_fused"]["kv_read_GBs"] = round(w.layer_hist_kv_bytes() / af / 1e6, 1)
+    sweep_on = rank == 0 and world == 1 and not args.no_sweep and args.workload == "lwm_5k"
+    if sweep_on:
+        line["overlap_f4"] = {args.workload: measure_overlap(w, lambda fn, n: timed_fn(fn, n, xs), 10)}
     w.sess.close()
     del w
     torch.cuda.empty_cache()
 
     # ---- the other full-size configs of BASELINE.json, same protocol, fewer steps (rank 0 of a 1-GPU run) ----
-    if rank == 0 and world == 1 and not args.no_sweep and args.workload == "lwm_5k":
-        line["sweep"] = run_sweep(args, device, timed, profile, pk, local)
+    if sweep_on:
+        line["sweep"] = run_sweep(args, device, timed, profile, pk, local, timed_fn, line["overlap_f4"])
+        line["decode"] = run_decode(args, device, timed, profile, pk)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
 
-def run_sweep(args, device, timed, profile, pk, local) -> dict:
+def run_decode(args, device, timed, profile, pk) -> dict:
+    """n = 1 (one decode step of one conversation) over the same pools: the path degenerates to a paged
+    read of the whole history per layer, so the roofline is HBM (history KV bytes / attention time)."""
+    import torch
+    from paper_2606_16135_b200 import binding as sc
+    out = {}
+    for name in ("lwm_5k", "lwm_50k"):
+        w = Workload(name, device, args.engine, args.copy, keep_host_layers=0, n_new=1)
+        e = {"workload": workload_string(name, w.shape, n_new=1)}
+        for m, mname in ((sc.SC_ATTN_STAGED, "staged"), (sc.SC_ATTN_FUSED, "fused")):
+            for _ in range(3):
+                w.turn(m)
+            steps = 20
+            ms = timed(w, m, steps) / steps
+            prof = profile(w, m, 2)
+            att = _avg(prof["attention"])
+            e[mname] = {"ms_per_step": round(ms, 4), "kv_gbs": round(w.layer_hist_kv_bytes() * w.shape.L / ms / 1e6, 1),
+                        "attention_avg_ms": round(att, 5) if att else None,
+                        "attention_kv_read_GBs": round(w.layer_hist_kv_bytes() / att / 1e6, 1) if att else None,
+                        "frac_of_measured_hbm": round(w.layer_hist_kv_bytes() / att / 1e6 / pk["hbm_gbs"], 4) if att else None}
+        out[name] = e
+        w.sess.close()
+        del w
+        torch.cuda.empty_cache()
+    return out
+
+
+def run_sweep(args, device, timed, profile, pk, local, timed_fn, overlap) -> dict:
     """lwm_50k, gqa_128k (HBM and pinned-host pool), multiturn (turns 0 and 9): ms per turn in both
     modes, per-kernel averages against the measured peaks, clocks sampled during each timed region."""
     import torch
@@ -652,6 +778,8 @@ def run_sweep(args, device, timed, profile, pk, local) -> dict:
             g = entry["staged"]["kernels"].get("gather", {})
             entry["pcie"] = {"pinned_memcpy_h2d_GBs": round(h2d_rate, 2), "gather_pool_read_GBs": g.get("pool_read_GBs"),
                              "frac_of_memcpy_rate": round(g["pool_read_GBs"] / h2d_rate, 4) if g.get("pool_read_GBs") else None}
+        if name in ("lwm_50k", "gqa_128k_host"):   # f4 over a long HBM history and over the host pool
+            overlap[name] = measure_overlap(w, lambda fn, n: timed_fn(fn, n, w.sess.compute_stream), 2 if host else 4)
         if shape.turns > 1:                         # config 5: ten successive turns; turn 0 above, now the last one
             entry["turn"] = 0
             for t in range(1, shape.turns):
