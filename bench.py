@@ -46,6 +46,8 @@ def parse_args():
     ap.add_argument("--copy", default="auto", choices=["auto", "ldg", "bulk"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--pool", default="config", choices=["config", "peer"],
+                    help="peer (needs --gpus 2): the pool lives on rank 1's GPU, rank 0 reads it over NVLink (f2)")
     ap.add_argument("--no-sweep", action="store_true", help="only the headline workload")
     ap.add_argument("--sweep", default=",".join(SWEEP), help="comma-separated workloads measured beside the headline")
     return ap.parse_args()
@@ -133,7 +135,7 @@ def workload_string(name: str, shape, n_new=None) -> str:
 class Workload:
     """Synthetic conversations of one BASELINE.json config, resident in HBM."""
 
-    def __init__(self, name: str, device, engine="auto", copy="auto", keep_host_layers=1, n_new=None):
+    def __init__(self, name: str, device, engine="auto", copy="auto", keep_host_layers=1, n_new=None, peer_pool_ptr=None):
         import torch
         from paper_2606_16135_b200 import binding as sc
         from paper_2606_16135_b200 import inputs as I
@@ -150,9 +152,11 @@ class Workload:
         blocks = [-(-(h + n * shape.turns) // B) for h, n in zip(self.hist, self.n_new)]   # room for every turn
         self.max_blocks = max(blocks)
         pool_kind = sc.SC_POOL_HOST_PINNED if shape.pool_kind == "host" else sc.SC_POOL_HBM
+        if peer_pool_ptr is not None:          # f2: the region is another GPU's memory, mapped by the caller
+            pool_kind = sc.SC_POOL_PEER
         self.sess = Session(shape.L, shape.Hq, shape.Hkv, shape.D, B, shape.n_blocks, sum(blocks),
                             int(self.cu[-1]), max_seqs=self.n_seq, pool_kind=pool_kind,
-                            alloc_seed=I.BASE_SEED + shape.config_id, device=device)
+                            alloc_seed=I.BASE_SEED + shape.config_id, device=device, pool_ptr=peer_pool_ptr)
         eng = {"auto": sc.SC_ENGINE_AUTO, "mma": sc.SC_ENGINE_MMA_SYNC, "tcgen05": sc.SC_ENGINE_TCGEN05}[engine]
         cpy = {"auto": sc.SC_COPY_AUTO, "ldg": sc.SC_COPY_LDG, "bulk": sc.SC_COPY_BULK}[copy]
         self.sess.pool.set_engine(eng, cpy)
@@ -422,6 +426,43 @@ def pinned_h2d_rate(torch, device, mb=1024) -> float:
     return best
 
 
+def peer_pool(args, world: int, rank: int, local: int):
+    """with `--gpus 2 --pool peer` the pool region is allocated on rank 1's GPU and
+    opened on rank 0 through CUDA IPC (one process per GPU); rank 0 then runs the workload with
+    pool_kind = SC_POOL_PEER, i.e. every pool read and write crosses NVLink, and rank 1 only lends the
+    memory.  Returns (pointer valid on this rank's device or None, keep-alive objects).
+    UNMEASURED by the builder: it needs two GPUs."""
+    import torch
+    import torch.distributed as dist
+    from cuda import cudart
+    from paper_2606_16135_b200 import binding as sc
+    from paper_2606_16135_b200 import inputs as I
+    shape = I.configs()[args.workload]
+    blocks = sum(-(-(h + shape.n_new * shape.turns) // shape.B) for h in shape.hist)
+    cfg = sc.make_config(shape.L, shape.Hq, shape.Hkv, shape.D, shape.B, shape.n_blocks, blocks, shape.n_new)
+    pool_bytes, _ = sc.sc_pool_bytes_required(cfg)
+    keep, payload = [], [None]
+    if rank == 1:
+        mem = torch.zeros(pool_bytes + 1024, dtype=torch.uint8, device=f"cuda:{local}")
+        err, handle = cudart.cudaIpcGetMemHandle(mem.data_ptr())
+        if int(err) != 0:
+            raise SystemExit(f"cudaIpcGetMemHandle: {err}")
+        payload = [(bytes(handle.reserved), mem.data_ptr() % 1024)]
+        keep.append(mem)
+    dist.broadcast_object_list(payload, src=1)
+    ptr = None
+    if rank == 0:
+        raw, mis = payload[0]
+        h = cudart.cudaIpcMemHandle_t()
+        h.reserved = raw
+        err, base = cudart.cudaIpcOpenMemHandle(h, cudart.cudaIpcMemLazyEnablePeerAccess)
+        if int(err) != 0:
+            raise SystemExit(f"cudaIpcOpenMemHandle: {err} (is there a P2P path between the two GPUs?)")
+        ptr = int(base) + (-(int(base) + 0)) % 1024
+        keep.append(base)
+    return ptr, keep
+
+
 class Filler:
     """The work a model does between two attentions -- o-proj, FFN (gate, up, down) of layer l and the
     QKV projection of layer l+1 for the turn's new tokens, Llama-2-7B sizes, random weights -- as ONE
@@ -565,7 +606,17 @@ def run_ours(args):
         return prof
 
     STAGED, FUSED = sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED
-    w = Workload(args.workload, device, args.engine, args.copy)
+    peer_ptr, peer_keep = None, None
+    if args.pool == "peer":
+        if world != 2:
+            raise SystemExit("--pool peer needs exactly two ranks (torchrun --nproc-per-node 2 ... --gpus 2)")
+        peer_ptr, peer_keep = peer_pool(args, world, rank, local)
+        if rank == 1:                          # lends its memory and waits for rank 0
+            dist.barrier()
+            dist.destroy_process_group()
+            return
+        world = 1                              # one conversation, one compute GPU: no max-over-ranks below
+    w = Workload(args.workload, device, args.engine, args.copy, peer_pool_ptr=peer_ptr)
     shape, pool, xs = w.shape, w.sess.pool, w.sess.compute_stream
     mode = STAGED if args.mode == "staged" else FUSED
 
@@ -674,10 +725,11 @@ def run_ours(args):
     kv_turn_bytes = w.layer_hist_kv_bytes() * shape.L
     job = whole_job(ms_per_step, world, kv_turn_bytes, w.layer_flops() * shape.L)
     line = {
-        "metric": METRIC, "value": round(ms_per_step, 4), "unit": "ms", "n_gpus": world, "steps": args.steps,
+        "metric": METRIC, "value": round(ms_per_step, 4), "unit": "ms", "n_gpus": 2 if peer_ptr else world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": config_dict(args.workload, shape, args.mode, world),
+        "pool": ("peer GPU over NVLink (CUDA IPC, SC_POOL_PEER); link rate ~900 GB/s per direction" if peer_ptr else shape.pool_kind),
         "kv_gbs": round(job["kv_gbs"], 1),
         "attn_tflops": round(job["attn_tflops"], 1),
         "other_mode": {"mode": "fused" if other_mode == FUSED else "staged", "value": round(other_ms, 4),
@@ -694,7 +746,7 @@ def run_ours(args):
     if af:
         line["isolated"]["attention_fused"]["TFLOPs"] = round(w.layer_flops() / af / 1e9, 1)
         line["isolated"]["attention_fused"]["kv_read_GBs"] = round(w.layer_hist_kv_bytes() / af / 1e6, 1)
-    sweep_on = rank == 0 and world == 1 and not args.no_sweep and args.workload == "lwm_5k"
+    sweep_on = rank == 0 and world == 1 and not args.no_sweep and args.workload == "lwm_5k" and not peer_ptr
     if sweep_on:
         line["overlap_f4"] = {args.workload: measure_overlap(w, lambda fn, n: timed_fn(fn, n, xs), 10)}
     w.sess.close()
@@ -707,7 +759,10 @@ def run_ours(args):
         line["decode"] = run_decode(args, device, timed, profile, pk)
     if rank == 0:
         print(json.dumps(line))
-    if world > 1:
+    if peer_ptr:
+        dist.barrier()                         # releases rank 1
+        dist.destroy_process_group()
+    elif world > 1:
         dist.destroy_process_group()
 
 

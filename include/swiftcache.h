@@ -65,7 +65,13 @@ typedef enum {
     SC_ERR_UNSUPPORTED = 6    /* head_dim not in {64,128}, block_size != 16, Hq % Hkv != 0  */
 } sc_status_t;
 
-typedef enum { SC_POOL_HBM = 0, SC_POOL_HOST_PINNED = 1 } sc_pool_kind_t;
+/* where the pool region lives.  SC_POOL_PEER: the memory of ANOTHER GPU --
+ * the paper's actual donor, "the worker GPU's idle memory ... accessed over NVLink" (PAPER.md:132,
+ * :148, :332) -- mapped into this process by the caller (cudaDeviceEnablePeerAccess for a
+ * same-process allocation, cudaIpcOpenMemHandle for another process's); every kernel addresses the
+ * pool through pool_base only, so gather, scatter and fused attention read and write it across the
+ * link exactly as they do local HBM.  The LSC is always local. */
+typedef enum { SC_POOL_HBM = 0, SC_POOL_HOST_PINNED = 1, SC_POOL_PEER = 2 } sc_pool_kind_t;
 typedef enum { SC_ATTN_STAGED = 0, SC_ATTN_FUSED = 1 } sc_attn_mode_t;
 typedef enum { SC_MEM_DEVICE = 0, SC_MEM_HOST_PINNED = 1 } sc_mem_kind_t;
 /* which attention engine sc_prefill_layer* uses; AUTO picks the fastest one
@@ -110,8 +116,8 @@ const char *sc_last_error(void);
  * LSC buffers).  Pure host arithmetic (Eq. 1); works without a GPU.  HOST pointers. */
 sc_status_t sc_pool_bytes_required(const sc_pool_config_t *cfg, size_t *pool_bytes, size_t *lsc_bytes);
 
-/* pool_base: DEVICE pointer (SC_POOL_HBM) or pinned, device-mapped HOST pointer
- * (SC_POOL_HOST_PINNED), 1024-byte aligned, >= pool_bytes.  lsc_base: DEVICE pointer,
+/* pool_base: DEVICE pointer (SC_POOL_HBM), peer-DEVICE pointer valid on the current device
+ * (SC_POOL_PEER) or pinned, device-mapped HOST pointer (SC_POOL_HOST_PINNED), 1024-byte aligned, >= pool_bytes.  lsc_base: DEVICE pointer,
  * 1024-byte aligned, >= lsc_bytes; may be NULL with lsc_blocks == 0 (fused mode only).
  * If zero_fill != 0 both regions are cleared; this is optional: the data path never
  * relies on what a slot it did not write holds (S10: the scatter of a turn zero-fills

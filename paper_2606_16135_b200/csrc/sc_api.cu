@@ -51,7 +51,7 @@ sc_status_t make_geom(const sc_pool_config_t *c, ScGeom *g)
     if (c->n_q_heads % c->n_kv_heads)
         return sc_fail(SC_ERR_UNSUPPORTED, "n_q_heads %d not a multiple of n_kv_heads %d", c->n_q_heads,
                     c->n_kv_heads);
-    if (c->pool_kind != SC_POOL_HBM && c->pool_kind != SC_POOL_HOST_PINNED)
+    if (c->pool_kind != SC_POOL_HBM && c->pool_kind != SC_POOL_HOST_PINNED && c->pool_kind != SC_POOL_PEER)
         return sc_fail(SC_ERR_INVALID_ARG, "pool_kind %d", c->pool_kind);
     g->L = c->n_layers; g->Hq = c->n_q_heads; g->Hkv = c->n_kv_heads; g->D = c->head_dim;
     g->B = c->block_size; g->nh = c->head_dim / 64;

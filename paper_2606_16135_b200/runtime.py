@@ -33,7 +33,10 @@ class Session:
     """One pool + LSC + two streams on one GPU."""
 
     def __init__(self, L, Hq, Hkv, D, B, n_blocks, lsc_blocks, max_new_tokens, max_seqs=1,
-                 pool_kind=sc.SC_POOL_HBM, alloc_seed=0, device="cuda:0", zero_fill=True, fill_byte=None):
+                 pool_kind=sc.SC_POOL_HBM, alloc_seed=0, device="cuda:0", zero_fill=True, fill_byte=None,
+                 pool_ptr=None):
+        """`pool_ptr`: address of a pool region the caller already owns and has mapped on `device`
+        (SC_POOL_PEER: another GPU's memory); otherwise the session allocates the region itself."""
         if not torch.cuda.is_available():
             raise RuntimeError("swiftcache needs a CUDA device (no CPU fallback)")
         self.device = torch.device(device)
@@ -41,13 +44,17 @@ class Session:
         self.cfg = sc.make_config(L, Hq, Hkv, D, B, n_blocks, lsc_blocks, max_new_tokens, max_seqs,
                                   pool_kind, alloc_seed)
         pool_bytes, lsc_bytes = sc.sc_pool_bytes_required(self.cfg)
-        self.pool_mem, self._pool_owner = _aligned_bytes(
-            pool_bytes, self.device, pinned=(pool_kind == sc.SC_POOL_HOST_PINNED))
+        if pool_ptr is None:
+            self.pool_mem, self._pool_owner = _aligned_bytes(
+                pool_bytes, self.device, pinned=(pool_kind == sc.SC_POOL_HOST_PINNED))
+            pool_ptr = self.pool_mem.data_ptr()
+        else:
+            self.pool_mem = self._pool_owner = None
         self.lsc_mem, self._lsc_owner = _aligned_bytes(max(lsc_bytes, 1024), self.device)
         if fill_byte is not None:          # tests: what the borrowed memory holds before the pool exists
             self.pool_mem.fill_(fill_byte)
             self.lsc_mem.fill_(fill_byte)
-        self.pool = sc.Pool(self.cfg, self.pool_mem.data_ptr(), pool_bytes,
+        self.pool = sc.Pool(self.cfg, pool_ptr, pool_bytes,
                             self.lsc_mem.data_ptr() if lsc_blocks else 0, lsc_bytes, zero_fill=zero_fill)
         self.L, self.Hq, self.Hkv, self.D, self.B = L, Hq, Hkv, D, B
         # the compute stream outranks the copy stream: when an SM frees up, an attention CTA (which

@@ -98,3 +98,22 @@ def test_scale_decisions_drive_a_resize_in_whole_units():
     p.resize(64 - bw)
     assert p.num_free_blocks() == 32
     p.destroy()
+
+
+def test_layer_major_would_move_what_block_major_does_not():
+    """PAPER.md:208-216 (Fig. 6): in a layer-major pool [L][n_blocks] the slab of layer l starts at
+    l * n_blocks * cell; growing n_blocks -> n_blocks' shifts the slab of every layer l >= 1, i.e.
+    (L - 1) * n_blocks cells must be copied -- O(n_layers * n_blocks).  The block-major pool of this
+    library moves nothing: the offset of every surviving (block, layer) cell is unchanged."""
+    L, nb, nb2 = 32, 384, 400
+    c = sc.make_config(L, 32, 32, 128, 16, nb, 0, 16)
+    p = sc.Pool(c)                                            # host-only
+    cell = p.info().cell_bytes
+    probe = [(b, l) for b in (0, 1, nb // 2, nb - 1) for l in (0, 1, L // 2, L - 1)]
+    before = [p.cell_offset(b, l, 0, 0, 0, 0) for b, l in probe]
+    p.resize(nb2)
+    assert [p.cell_offset(b, l, 0, 0, 0, 0) for b, l in probe] == before         # block-major: 0 bytes moved
+    layer_major = lambda n, b, l: (l * n + b) * cell                              # noqa: E731
+    moved = sum(cell for l in range(L) for b in range(nb) if layer_major(nb, b, l) != layer_major(nb2, b, l))
+    assert moved == (L - 1) * nb * cell == 31 * 384 * 256 * 1024                  # 2.9 GiB for 16 more blocks
+    p.destroy()

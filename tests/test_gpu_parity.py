@@ -242,3 +242,46 @@ def test_pool_and_lsc_prefilled_with_nan(engine, T_h, n, split_tiles):
         assert np.array_equal(torch_to_bits(k), np.concatenate([c.data[0][1], c.data[0][3]]))
         assert np.array_equal(torch_to_bits(v), np.concatenate([c.data[0][2], c.data[0][4]]))
         c.close()
+
+
+# ------------------------------------------------------------------ f2: a pool behind a peer pointer
+def test_peer_pool_kind_routes_like_hbm():
+    """the donor pool is another GPU's memory,
+    mapped by the caller and handed over as pool_base with pool_kind = SC_POOL_PEER.  One GPU is
+    all a test can have, so the "peer" region here is a second local allocation the session does
+    not own; what is checked is that every call takes the pointer as it is: store, gather,
+    scatter, staged and fused attention against the oracle, and the raw bytes of the region."""
+    L, Hq, Hkv, D, B, NB, T_h, n = 2, 8, 2, 128, 16, 48, 333, 70
+    cfg = sc.make_config(L, Hq, Hkv, D, B, NB, 32, n, pool_kind=sc.SC_POOL_PEER)
+    pool_bytes, _ = sc.sc_pool_bytes_required(cfg)
+    region = torch.full((pool_bytes + 1024,), 0xFF, dtype=torch.uint8, device="cuda")    # never cleared: NaN bits
+    ptr = region.data_ptr() + (-region.data_ptr()) % 1024
+    sess = Session(L, Hq, Hkv, D, B, NB, 32, n, pool_kind=sc.SC_POOL_PEER, pool_ptr=ptr, zero_fill=False)
+    table = I.block_table(3, NB, O.blocks_for(T_h + n, B))
+    tdev = sess.table_dev(table)
+    opool = O.Pool(L, Hkv, D, B, NB)
+    st = torch.cuda.current_stream().cuda_stream
+    for l in range(L):
+        q, kh, vh, kn, vn = I.make_qkv(n, T_h, Hq, Hkv, D, 4242 + l)
+        sess.store_prefix(l, bits_to_torch(kh, sess.device), bits_to_torch(vh, sess.device), 0, tdev)
+        opool.store(l, 0, kh, 0, table)
+        opool.store(l, 1, vh, 0, table)
+        ref = O.prefill_layer(opool, l, q, kn, vn, table, T_h)
+        dq, dk, dv = (bits_to_torch(x, sess.device) for x in (q, kn, vn))
+        for mode in (sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED):
+            out = torch.zeros((n, Hq, D), dtype=torch.bfloat16, device=sess.device)
+            if mode == sc.SC_ATTN_STAGED:
+                sess.pool.load_layer(l, tdev.data_ptr(), len(table), T_h, l & 1, st)
+            sess.pool.prefill_layer(l, dq.data_ptr(), dk.data_ptr(), dv.data_ptr(), tdev.data_ptr(), len(table),
+                                    T_h, n, l & 1, mode, out.data_ptr(), st)
+            torch.cuda.synchronize()
+            assert_close(torch_to_bits(out), ref, f"peer pool, layer {l} mode {mode}")
+        k, v = sess.read_tokens(l, 0, tdev, 0, T_h + n)
+        assert np.array_equal(torch_to_bits(k), opool.gather(l, 0, table, T_h + n))
+        assert np.array_equal(torch_to_bits(v), opool.gather(l, 1, table, T_h + n))
+    # the bytes are in the caller's region, where sc_cell_offset says
+    raw = region.cpu().numpy()[ptr - region.data_ptr():].view(np.uint16)
+    t, h, d = 350, 1, 77
+    off = sess.pool.cell_offset(int(table[t // 16]), 1, 0, h, t % 16, d)
+    assert raw[off // 2] == opool.gather(1, 0, table, T_h + n)[t, h, d]
+    sess.close()

@@ -326,3 +326,78 @@ def test_block_major_resize_on_the_device():
         k, v = read(l, tdev, 6, 0, T)
         assert torch.equal(k.view(torch.int16), ks[l].view(torch.int16))
     p.destroy()
+
+
+def test_elastic_exchange_between_master_and_worker_pools():
+    """f1, both sides of the exchange ("whenever the master scales by MEU_m blocks the
+    i-th worker must simultaneously scale by MEU_i").  One borrowed region is the memory budget of a
+    worker GPU; an LWM-1M-Text-shaped master pool (32 layers x 32 kv heads: 8 MiB per block) and a
+    Qwen3-14B-shaped worker pool (40 layers x 8 kv heads: 2.5 MiB per block) are carved from it.
+    sc_scale_up's answer drives sc_pool_resize on BOTH: the worker gains d_worker blocks, the
+    master gives up d_master; the two byte counts are equal to the byte (MEU_m * BE_m = MEU_i * BE_i,
+    Eq. 8-9), so the budget is conserved, and neither pool moves a block: both conversations read
+    back bit-exactly through their old tables, the worker's new blocks are usable at once."""
+    mcfg = sc.make_config(32, 32, 32, 128, 16, 15, 0, 64)
+    wcfg = sc.make_config(40, 32, 8, 128, 16, 16, 0, 64)
+    meu_m, meu_w = sc.sc_elastic_units(mcfg, wcfg)
+    assert (meu_m, meu_w) == (5, 16)
+    m_bytes, _ = sc.sc_pool_bytes_required(mcfg)
+    w_bytes, _ = sc.sc_pool_bytes_required(wcfg)
+    bbm, bbw = m_bytes // 15, w_bytes // 16
+    assert meu_m * bbm == meu_w * bbw == 40 << 20                  # one elastic unit: the same 40 MiB on both sides
+    # the worker's share starts where the master's 15 blocks end and has room for the unit it may gain
+    region = torch.empty(m_bytes + w_bytes + meu_w * bbw + 1024, dtype=torch.uint8, device="cuda")
+    base = region.data_ptr() + (-region.data_ptr()) % 1024
+    master = sc.Pool(mcfg, base, m_bytes, 0, 0)
+    worker = sc.Pool(wcfg, base + m_bytes, w_bytes, 0, 0)
+    budget = master.info().pool_bytes + worker.info().pool_bytes
+
+    def fill(pool, cfg_, n_blocks, seed):
+        ids = pool.alloc_blocks(n_blocks)
+        tdev = torch.from_numpy(ids.copy()).cuda()
+        T = n_blocks * 16 - 3
+        data = {}
+        for l in (0, cfg_.n_layers - 1):
+            k = bits_to_torch(I.normal_bf16((T, cfg_.n_kv_heads, 128), seed + l), "cuda")
+            v = bits_to_torch(I.normal_bf16((T, cfg_.n_kv_heads, 128), seed + 50 + l), "cuda")
+            pool.store_prefix(l, k.data_ptr(), v.data_ptr(), 0, T, tdev.data_ptr(), len(ids))
+            data[l] = (k, v)
+        torch.cuda.synchronize()
+        return ids, tdev, T, data
+
+    def check(pool, cfg_, tdev, T, data):
+        for l, (k, v) in data.items():
+            ko, vo = torch.empty_like(k), torch.empty_like(v)
+            pool.read_tokens(l, 0, tdev.data_ptr(), tdev.numel(), 0, 0, T, ko.data_ptr(), vo.data_ptr())
+            torch.cuda.synchronize()
+            assert torch.equal(ko.view(torch.int16), k.view(torch.int16))
+            assert torch.equal(vo.view(torch.int16), v.view(torch.int16))
+
+    m_ids, m_t, m_T, m_data = fill(master, mcfg, 8, 700)           # ids 0..7: the master's tail stays free
+    w_ids, w_t, w_T, w_data = fill(worker, wcfg, 16, 900)          # the worker is full
+    # a 400-token request arrives at the worker: it holds 16 blocks, needs 25
+    d_w, d_m = sc.sc_scale_up(16, 16, meu_w, meu_m, 400)
+    assert (d_w, d_m) == (16, 5) and d_w * bbw == d_m * bbm
+    master.resize(15 - d_m)                                        # releases blocks 10..14 (free), moves nothing
+    worker.resize(16 + d_w, w_bytes + d_w * bbw)                   # appends blocks 16..31
+    assert master.info().pool_bytes + worker.info().pool_bytes == budget
+    assert m_bytes - master.info().pool_bytes == worker.info().pool_bytes - w_bytes == d_m * bbm
+    check(master, mcfg, m_t, m_T, m_data)
+    check(worker, wcfg, w_t, w_T, w_data)
+    new_ids, n_t, n_T, n_data = fill(worker, wcfg, d_w, 1100)      # the new blocks hold a second conversation
+    assert sorted(new_ids.tolist()) == list(range(16, 32))
+    check(worker, wcfg, n_t, n_T, n_data)
+    check(worker, wcfg, w_t, w_T, w_data)
+    with pytest.raises(sc.SwiftCacheError):
+        master.cell_offset(10, 0, 0, 0, 0, 0)                      # gone from the master
+    # and back: the request is gone, nothing longer than 250 tokens was seen lately
+    worker.free_blocks(new_ids)
+    b_w, b_m = sc.sc_scale_down(32, 16, meu_w, meu_m, 250)
+    assert (b_w, b_m) == (16, 5)
+    worker.resize(32 - b_w)
+    master.resize(10 + b_m, m_bytes)
+    assert master.info().pool_bytes + worker.info().pool_bytes == budget
+    check(master, mcfg, m_t, m_T, m_data)
+    check(worker, wcfg, w_t, w_T, w_data)
+    master.destroy()
+    worker.destroy()
