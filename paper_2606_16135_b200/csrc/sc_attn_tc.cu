@@ -374,6 +374,18 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     const uint32_t bar_recv = smem_u32(&bars->recv);
     const uint32_t q_smem = base + P::kQOff, ring = base + P::kRingOff;
 
+    // Producer warp, lanes 0-7: where block (tile's first block + lane) of this sequence lives.  The
+    // block-table read of the FIRST tile is issued here, before the set-up barriers, so that its
+    // latency (all CTAs of a launch hit the same table lines at once) is off the critical path.
+    auto block_ptr = [&](int tb) -> const char * {
+        const int lb = min(tb + lane, b_end - 1);
+        // a resident block (regular cache) is read in place, the rest from the LSC
+        return (a.has_res && lb < b.rc_blk[s])
+                   ? a.kv_res.base + sc_phys_block(a.kv_res, b, s, lb) * a.kv_res.block_stride
+                   : a.kv.base + sc_phys_block(a.kv, b, s, lb) * a.kv.block_stride;
+    };
+    const char *blk_next = (warp == 0 && lane < kTileBlks) ? block_ptr(b_begin) : nullptr;
+
     if (threadIdx.x == 0) {
         for (int i = 0; i < kStages; ++i) { mbar_init(bar_full + 8 * i, 1); mbar_init(bar_empty + 8 * i, 1); }
         for (int m = 0; m < 2; ++m) {
@@ -398,6 +410,8 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     // Programmatic dependent launch: everything above overlapped the tail of the kernel before this
     // one in the stream; nothing below may start until that kernel's memory is visible (q, k_new,
     // v_new of this layer come from it in a model).  Then let the NEXT kernel begin its own set-up.
+    // (Moving the wait to the top of the kernel, to start the Q loads earlier, was measured: it gives
+    // up the overlap of the set-up with the previous kernel's tail, 1.18 -> 1.31 ms per fused turn.)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (threadIdx.x == 128) TL(1);
@@ -479,39 +493,36 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     else asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
     if (warp == 0) {
         // =============================== producer ===============================
-        if (lane == 0) {
+        // Lane 0 owns the ring protocol (waits for a free slot, arms the full barrier); lanes 0-7 each
+        // look up ONE block of the tile in the block table and issue its two bulk copies, and read
+        // the table for the next tile while this one's copies are in flight.
+        {
             const int hk = h / (g.Hq / g.Hkv);
             const int64_t off_kv[2] = {(int64_t)hk * P::kChunk, (int64_t)(g.Hkv + hk) * P::kChunk};
             bool scat_waited = (a.k_new == nullptr);
             for (int jj = 0; jj < nt_max; ++jj) {
                 const int tb = b_begin + jj * kTileBlks;         // first block of the tile
                 const int nbt = min(kTileBlks, b_end - tb);      // blocks it holds
+                const char *blk = blk_next;
+                if (jj + 1 < nt_max && lane < kTileBlks) blk_next = block_ptr(tb + kTileBlks);
                 if (!scat_waited && tb + nbt > (T_h >> 4)) {     // first tile with a block the scatter touches
-                    mbar_wait_cluster(bar_scat, 0);
+                    if (lane == 0) mbar_wait_cluster(bar_scat, 0);
+                    __syncwarp();
                     asm volatile("fence.proxy.async.global;" ::: "memory");   // generic-proxy stores -> bulk-copy reads
                     scat_waited = true;
-                }
-                const char *blk[kTileBlks];
-#pragma unroll
-                for (int c = 0; c < kTileBlks; ++c) {
-                    const int lb = min(tb + c, b_end - 1);
-                    // a resident block (regular cache) is read in place, the rest from the LSC
-                    blk[c] = (a.has_res && lb < b.rc_blk[s])
-                                 ? a.kv_res.base + sc_phys_block(a.kv_res, b, s, lb) * a.kv_res.block_stride
-                                 : a.kv.base + sc_phys_block(a.kv, b, s, lb) * a.kv.block_stride;
                 }
 #pragma unroll
                 for (int kv = 0; kv < 2; ++kv) {
                     const int it = 2 * jj + kv, slot = it % kStages;
-                    mbar_wait(bar_empty + 8 * slot, ((it / kStages) & 1) ^ 1);
-                    if (PROBE(4)) { mbar_arrive(bar_full + 8 * slot); continue; }
-                    mbar_expect_tx(bar_full + 8 * slot, (uint32_t)nbt * P::kChunk);
-#pragma unroll
-                    for (int c = 0; c < kTileBlks; ++c)
-                        if (c < nbt)
-                            bulk_g2s(ring + slot * P::kSlot + c * P::kChunk, blk[c] + off_kv[kv], P::kChunk,
-                                     bar_full + 8 * slot);
-                    if (it == 0) {
+                    if (lane == 0) {
+                        mbar_wait(bar_empty + 8 * slot, ((it / kStages) & 1) ^ 1);
+                        if (PROBE(4)) mbar_arrive(bar_full + 8 * slot);
+                        else mbar_expect_tx(bar_full + 8 * slot, (uint32_t)nbt * P::kChunk);
+                    }
+                    __syncwarp();
+                    if (lane < nbt && !PROBE(4))
+                        bulk_g2s(ring + slot * P::kSlot + lane * P::kChunk, blk + off_kv[kv], P::kChunk, bar_full + 8 * slot);
+                    if (it == 0 && lane == 0) {
                         // The first MMA needs Q and K of tile 0 only.  All CTAs start together, so
                         // the rest of the ring is requested once Q has landed: it would only queue
                         // in front of Q at the memory controllers.

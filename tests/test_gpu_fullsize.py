@@ -115,6 +115,17 @@ def test_gqa_128k_sampled():
     w.sess.close()
 
 
+def test_gqa_128k_host_pool_sampled():
+    """Config 4, second variant: the same 131 072-token GQA history in a PINNED-HOST pool (the PCIe
+    reload path).  One staged turn: every layer's gather crosses PCIe into the LSC, the scatter
+    writes host memory; two layers x two heads x all rows against the oracle, pool bytes on the
+    device against the regenerated history."""
+    w = _workload("gqa_128k_host")
+    L, Hq = w.shape.L, w.shape.Hq
+    _check_turn(w, sc.SC_ATTN_STAGED, layers=[0, L - 1], heads=[0, Hq - 1], convs=[0], what="gqa_128k_host staged")
+    w.sess.close()
+
+
 def test_multiturn_ten_turns():
     """Config 5: 8 ragged conversations over one shared shuffled pool; ten successive turns,
     each turn's new KV scattered back and read by the next (I2 every turn, O6)."""
