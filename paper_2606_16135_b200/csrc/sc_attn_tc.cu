@@ -122,6 +122,13 @@ __device__ __forceinline__ void bulk_g2s(uint32_t smem_dst, const void *gsrc, ui
         "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
         :: "r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar) : "memory");
 }
+// the same with an L2 cache policy (createpolicy) for the lines it touches
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t smem_dst, const void *gsrc, uint32_t bytes, uint32_t bar, uint64_t pol)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+        :: "r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
 // this CTA's shared memory -> a peer CTA's shared memory (destination and barrier are addresses
 // in the shared::cluster window of the peer), completing on the PEER's mbarrier
 __device__ __forceinline__ void bulk_s2peer(uint32_t peer_dst, uint32_t src, uint32_t bytes, uint32_t peer_bar)
@@ -500,6 +507,9 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             const int hk = h / (g.Hq / g.Hkv);
             const int64_t off_kv[2] = {(int64_t)hk * P::kChunk, (int64_t)(g.Hkv + hk) * P::kChunk};
             bool scat_waited = (a.k_new == nullptr);
+            // staged mode: an LSC line is read exactly once per layer -- after that it may go first
+            uint64_t pol_stream = 0;
+            if (LEAN) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
             for (int jj = 0; jj < nt_max; ++jj) {
                 const int tb = b_begin + jj * kTileBlks;         // first block of the tile
                 const int nbt = min(kTileBlks, b_end - tb);      // blocks it holds
@@ -520,8 +530,10 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                         else mbar_expect_tx(bar_full + 8 * slot, (uint32_t)nbt * P::kChunk);
                     }
                     __syncwarp();
-                    if (lane < nbt && !PROBE(4))
-                        bulk_g2s(ring + slot * P::kSlot + lane * P::kChunk, blk + off_kv[kv], P::kChunk, bar_full + 8 * slot);
+                    if (lane < nbt && !PROBE(4)) {
+                        if (LEAN) bulk_g2s_hint(ring + slot * P::kSlot + lane * P::kChunk, blk + off_kv[kv], P::kChunk, bar_full + 8 * slot, pol_stream);
+                        else bulk_g2s(ring + slot * P::kSlot + lane * P::kChunk, blk + off_kv[kv], P::kChunk, bar_full + 8 * slot);
+                    }
                     if (it == 0 && lane == 0) {
                         // The first MMA needs Q and K of tile 0 only.  All CTAs start together, so
                         // the rest of the ring is requested once Q has landed: it would only queue
