@@ -425,10 +425,10 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     float fin_m = -INFINITY, fin_l = 0.f;      // softmax threads: final (m in log2 units, l) of their row
 
     // ---- scatter (a5) ----
-    // The pair's new tokens [T_h, T_h + ntok) are stored into the pool (and the LSC tail in staged
-    // mode); the CTA of a sequence's LAST pair also zero-fills the rest of the last block, so that
-    // slots past the logical end hold finite values whatever the memory held before (they are
-    // masked in S, but 0 * NaN in P.V would poison the row).
+    // Every slot from T_h on of the blocks the pair reads is stored into the pool (and the LSC tail in
+    // staged mode): the new tokens and, behind the sequence's last token, zeros, so that slots past the
+    // logical end hold finite values whatever the memory held before (they are masked in S, but
+    // 0 * NaN in P.V would poison the row).
     // Without a cluster (one CTA per pair): the softmax warps do it first, overlapped with the Q loads.
     // With a cluster (one CTA per split of this query pair and head): the rows are dealt out evenly
     // over the cluster's CTAs, whose otherwise idle warps 2-3 store them in the background, and each
@@ -440,9 +440,10 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         constexpr int NT = decltype(nthreads_c)::value;
         if (a.k_new == nullptr) { after_first_loads(); return; }
         bool mid_done = false;
-        const int ntok = min(n_s, tok0 + kPairM);                    // new tokens up to the end of this pair
-        const int npad = (tok0 + kPairM >= n_s) ? ((-(T_h + n_s)) & 15) : 0;
-        const int nall = ntok + npad;                                // rows of [K rows ; V rows] are 2 * nall
+        // every slot from T_h to the end of the last block this pair reads: the new tokens (up to 15 of
+        // the next pair, which share that block, included) and, behind the sequence's last token, zeros
+        const int ntok = n_s;
+        const int nall = 16 * need_max - T_h;                        // rows of [K rows ; V rows] are 2 * nall
         int rest_lo = 0, rest_hi = 2 * nall;
         if (a.cluster_combine) {
             const int per = (2 * nall + ns_act - 1) / ns_act;
