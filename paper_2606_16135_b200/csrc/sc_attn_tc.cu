@@ -434,8 +434,9 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     // over the cluster's CTAs, whose otherwise idle warps 2-3 store them in the background, and each
     // thread then arrives (release, cluster scope) on the scat_done barrier of every CTA of the
     // cluster; a producer waits for all of them before it loads the first KV tile that holds new
-    // tokens.  CTAs of other query heads of the group or of later query pairs may store the same
-    // bytes to the same places.
+    // tokens.  The host folds the scatter into this kernel only where that leaves ONE writer per row
+    // (no grouped-query heads, one query pair per sequence: sc_ops.cu); the code below does not rely
+    // on it.
     auto scatter_share = [&](auto nthreads_c, int tid, auto &&after_first_loads) {
         constexpr int NT = decltype(nthreads_c)::value;
         if (a.k_new == nullptr) { after_first_loads(); return; }

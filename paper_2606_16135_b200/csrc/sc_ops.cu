@@ -294,8 +294,13 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     if (n_splits == 1) cluster = false;
     // 1. scatter (a5): pool, and the LSC tail in staged mode.  The tcgen05 engine does it inside
     //    the attention kernel when a query pair's CTAs form a cluster (they share the work) or
-    //    when there is a single CTA per pair; otherwise the scatter kernel runs first.
-    const bool fold_scatter = tc && (cluster || n_splits == 1);
+    //    when there is a single CTA per pair -- but only where that makes ONE writer per row: no
+    //    grouped-query heads (the query heads of a group would each store the KV head's rows) and
+    //    one query pair per sequence (a later pair reads, and would store, the earlier pairs' rows).
+    //    Otherwise the scatter kernel runs first; it too writes every row once.
+    bool one_pair = true;
+    for (int i = 0; i < n_seq; ++i) one_pair = one_pair && (cu_new[i + 1] - cu_new[i] <= tile_m);
+    const bool fold_scatter = tc && (cluster || n_splits == 1) && pool->g.Hq == pool->g.Hkv && one_pair;
     if (!fold_scatter) {
         ScProfScope ps(pool, SC_KERNEL_SCATTER, s);
         SC_CUDA(sc_launch_scatter(pool->g, k_new, v_new, b, pv, staged ? &lv : nullptr, true, s));
