@@ -328,6 +328,7 @@ struct Bars {                       // at Plan::kBarOff
     uint64_t s_ready[2];            // MMA -> softmax warpgroup m: S_m written (and earlier PV_m done)
     uint64_t p_ready[2];            // softmax warpgroup m -> MMA: P_m stored, O_m rescaled
     uint64_t q_ready[2];            // Q_m in shared memory
+    uint64_t q_stage[2];            // the rows of Q_m have landed in their staging slot
     uint64_t scat_done;             // warps 2-3 -> producer: this CTA's share of the new K/V is in the pool
     uint64_t recv;                  // cluster epilogue: the peers' partials have landed in this CTA
     uint32_t tmem_base;
@@ -399,6 +400,7 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             mbar_init(bar_s + 8 * m, 1);
             mbar_init(bar_p + 8 * m, kTM);
             mbar_init(bar_q + 8 * m, kTM);
+            mbar_init(smem_u32(&bars->q_stage[m]), 1);
         }
         mbar_init(bar_scat, a.cluster_combine ? 64 * ns_act : 256);
         mbar_init(bar_recv, 1);
@@ -623,34 +625,36 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         const int row0 = tok0 + m * kTM;                      // first new-token index of the tile
         const int64_t grow = (int64_t)b.cu_new[s] + row0 + r; // packed row of (s, token)
         {
-            // ---- Q_m -> shared memory, swizzled exactly like a K tile; its global loads and the
-            //      first round of scatter loads share one memory round trip ----
+            // ---- Q_m -> shared memory, swizzled exactly like a K tile.  The rows travel by the TMA engine
+            //      (one 2*D-byte bulk copy per row, issued by the thread that owns the row) into ring slot
+            //      1 + m, which the producer does not use before Q has landed; the warpgroup then moves them
+            //      into place.  (Through the LSU path the 64 KB of Q took ~5k cycles: every SM starts
+            //      streaming K/V at the same moment, and an SM's pending-request capacity over the loaded
+            //      latency is ~11 B/clk.) ----
             constexpr int CPR = D / 8;                        // 16-byte units per row
-            const char *qg = (const char *)a.q;
             const uint32_t qs = q_smem + m * P::kQTile;
-            int4 qv[CPR];
+            const uint32_t stage = ring + (1 + m) * P::kSlot, bar_qs = smem_u32(&bars->q_stage[m]);
             if (nt[m] > 0) {
-#pragma unroll
-                for (int it = 0; it < CPR; ++it) {
-                    const int u = it * kTM + t128;
-                    const int row = u / CPR, c16 = u % CPR;
-                    qv[it] = make_int4(0, 0, 0, 0);
-                    if (row < rows[m])
-                        qv[it] = __ldg(reinterpret_cast<const int4 *>(
-                            qg + (((int64_t)b.cu_new[s] + row0 + row) * g.Hq + h) * (D * 2) + c16 * 16));
-                }
+                if (t128 == 0) mbar_expect_tx(bar_qs, (uint32_t)rows[m] * (D * 2));
+                if (r < rows[m])
+                    bulk_g2s(stage + r * (D * 2), (const char *)a.q + (grow * g.Hq + h) * (D * 2), D * 2, bar_qs);
             }
             auto store_q = [&]() {
                 if (nt[m] > 0) {
+                    mbar_wait(bar_qs, 0);
 #pragma unroll
                     for (int it = 0; it < CPR; ++it) {
                         const int u = it * kTM + t128;
                         const int row = u / CPR, c16 = u % CPR, hf = c16 >> 3, c = c16 & 7;
+                        uint32_t v0 = 0, v1 = 0, v2 = 0, v3 = 0;
+                        if (row < rows[m])
+                            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                                         : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3) : "r"(stage + row * (D * 2) + c16 * 16));
                         const uint32_t dst = qs + (row >> 3) * (NH * 1024) + hf * 1024 + (row & 7) * 128 + ((c ^ (row & 7)) << 4);
                         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
-                                     :: "r"(dst), "r"(qv[it].x), "r"(qv[it].y), "r"(qv[it].z), "r"(qv[it].w) : "memory");
+                                     :: "r"(dst), "r"(v0), "r"(v1), "r"(v2), "r"(v3) : "memory");
                     }
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // before the MMAs read Q and before V of tile 0 lands on the staging slot
                     mbar_arrive(bar_q + 8 * m);
                     if (threadIdx.x == 128) TL(2);
                 }
