@@ -63,3 +63,24 @@ def test_lwm_layer_shape_tcgen05():
     for h in (0, 13, 31):
         assert_close(got[:, h], ref[:, h], f"head {h}")
     c.close()
+
+
+@pytest.mark.parametrize("Hq,Hkv,n,folded", [(4, 4, 200, True), (4, 4, 300, False), (8, 2, 200, False)])
+def test_scatter_is_folded_only_with_one_writer_per_row(Hq, Hkv, n, folded):
+    """The tcgen05 kernel stores the turn's new K/V itself only where that leaves ONE writer per row: no
+    grouped-query heads (each query head of a group would store the KV head's rows) and one query pair
+    per sequence (a later pair would store the earlier pair's rows).  Otherwise the scatter kernel runs
+    first -- one more launch.  Either way the pool holds the new tokens bit for bit afterwards."""
+    T_h = 700
+    c = Case(L=1, Hq=Hq, Hkv=Hkv, D=128, T_h=T_h, n=n, NB=80, seed=6100 + n + Hq, engine=sc.SC_ENGINE_TCGEN05)
+    before = c.sess.pool.launch_count()
+    got = c.run_layer(0, sc.SC_ATTN_FUSED)
+    launches = c.sess.pool.launch_count() - before
+    assert_close(got, c.oracle_layer(0), f"Hq={Hq} Hkv={Hkv} n={n}")
+    k, v = c.sess.read_tokens(0, 0, c.table_dev, 0, T_h + n)
+    from paper_2606_16135_b200.runtime import torch_to_bits
+    assert np.array_equal(torch_to_bits(k), np.concatenate([c.data[0][1], c.data[0][3]]))
+    assert np.array_equal(torch_to_bits(v), np.concatenate([c.data[0][2], c.data[0][4]]))
+    # attention alone when folded; scatter + attention (+ combine when the KV range was split) otherwise
+    assert (launches == 1) if folded else (launches >= 2), launches
+    c.close()
