@@ -135,7 +135,8 @@ def workload_string(name: str, shape, n_new=None) -> str:
 class Workload:
     """Synthetic conversations of one BASELINE.json config, resident in HBM."""
 
-    def __init__(self, name: str, device, engine="auto", copy="auto", keep_host_layers=1, n_new=None, peer_pool_ptr=None):
+    def __init__(self, name: str, device, engine="auto", copy="auto", keep_host_layers=1, n_new=None, peer_pool_ptr=None,
+                 sorted_table=False):
         import torch
         from paper_2606_16135_b200 import binding as sc
         from paper_2606_16135_b200 import inputs as I
@@ -156,7 +157,8 @@ class Workload:
             pool_kind = sc.SC_POOL_PEER
         self.sess = Session(shape.L, shape.Hq, shape.Hkv, shape.D, B, shape.n_blocks, sum(blocks),
                             int(self.cu[-1]), max_seqs=self.n_seq, pool_kind=pool_kind,
-                            alloc_seed=I.BASE_SEED + shape.config_id, device=device, pool_ptr=peer_pool_ptr)
+                            alloc_seed=0 if sorted_table else I.BASE_SEED + shape.config_id, device=device,
+                            pool_ptr=peer_pool_ptr)          # alloc_seed 0: ids in order (the locality best case)
         eng = {"auto": sc.SC_ENGINE_AUTO, "mma": sc.SC_ENGINE_MMA_SYNC, "tcgen05": sc.SC_ENGINE_TCGEN05}[engine]
         cpy = {"auto": sc.SC_COPY_AUTO, "ldg": sc.SC_COPY_LDG, "bulk": sc.SC_COPY_BULK}[copy]
         self.sess.pool.set_engine(eng, cpy)
@@ -408,22 +410,25 @@ def kernel_table(w: "Workload", prof: dict, p_steps: int, staged: bool, pk: dict
     return kernels
 
 
-def pinned_h2d_rate(torch, device, mb=1024) -> float:
-    """GB/s of a plain pinned cudaMemcpy host -> device, measured in this run: the link rate the
-    host-pool gather is held against."""
+def pinned_copy_rates(torch, device, mb=1024) -> tuple:
+    """GB/s of a plain pinned cudaMemcpy host -> device and device -> host, measured in this run: the
+    link rate the host-pool gather (reads: H2D direction) is held against."""
     h = torch.empty(mb << 20, dtype=torch.uint8).pin_memory()
     d = torch.empty(mb << 20, dtype=torch.uint8, device=device)
-    d.copy_(h, non_blocking=True)
-    torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    best = 0.0
-    for _ in range(3):
-        e0.record()
-        d.copy_(h, non_blocking=True)
-        e1.record()
+    rates = []
+    for dst, src in ((d, h), (h, d)):
+        dst.copy_(src, non_blocking=True)
         torch.cuda.synchronize()
-        best = max(best, (mb << 20) / e0.elapsed_time(e1) / 1e6)
-    return best
+        best = 0.0
+        for _ in range(3):
+            e0.record()
+            dst.copy_(src, non_blocking=True)
+            e1.record()
+            torch.cuda.synchronize()
+            best = max(best, (mb << 20) / e0.elapsed_time(e1) / 1e6)
+        rates.append(best)
+    return rates[0], rates[1]
 
 
 def peer_pool(args, world: int, rank: int, local: int):
@@ -630,6 +635,17 @@ def run_ours(args):
     launches = pool.launch_count() - l0
     clocks = clk.stop() if clk else None
     ms_per_step = total_ms / args.steps
+    # the same turns one by one (an event after every turn, no host synchronisation in between): median and min
+    n_each = max(3, min(args.steps, 20))
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(n_each + 1)]
+    barrier()
+    evs[0].record(xs)
+    for i in range(n_each):
+        w.turn(mode)
+        evs[i + 1].record(xs)
+    barrier()
+    each = [evs[i].elapsed_time(evs[i + 1]) for i in range(n_each)]
+    per_turn = {"median_ms": round(float(np.median(each)), 4), "min_ms": round(float(np.min(each)), 4), "turns": n_each}
 
     # the other variant of the path beside it (same workload, same timing protocol, fewer steps):
     # fused = attention reads pool blocks through the block table, no gather into the LSC
@@ -734,7 +750,7 @@ def run_ours(args):
         "attn_tflops": round(job["attn_tflops"], 1),
         "other_mode": {"mode": "fused" if other_mode == FUSED else "staged", "value": round(other_ms, 4),
                        "unit": "ms", "steps": o_steps},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        "per_turn": per_turn, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof, "kernels": kernels,
         "isolated": {k: {"avg_ms": round(_avg(v), 5)} for k, v in iso.items() if _avg(v) is not None},
         "cpu_baseline": cpu, "parity": parity,
@@ -800,7 +816,7 @@ def run_sweep(args, device, timed, profile, pk, local, timed_fn, overlap) -> dic
     from paper_2606_16135_b200 import binding as sc
     STAGED, FUSED = sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED
     out = {}
-    h2d_rate = None
+    h2d_rate = d2h_rate = None
     for name in [x for x in args.sweep.split(",") if x]:
         t_begin = time.perf_counter()
         try:
@@ -829,9 +845,11 @@ def run_sweep(args, device, timed, profile, pk, local, timed_fn, overlap) -> dic
 
         measure(entry)
         if host:
-            h2d_rate = h2d_rate or pinned_h2d_rate(torch, device)
+            if h2d_rate is None:
+                h2d_rate, d2h_rate = pinned_copy_rates(torch, device)
             g = entry["staged"]["kernels"].get("gather", {})
-            entry["pcie"] = {"pinned_memcpy_h2d_GBs": round(h2d_rate, 2), "gather_pool_read_GBs": g.get("pool_read_GBs"),
+            entry["pcie"] = {"pinned_memcpy_h2d_GBs": round(h2d_rate, 2), "pinned_memcpy_d2h_GBs": round(d2h_rate, 2),
+                             "gather_pool_read_GBs": g.get("pool_read_GBs"),
                              "frac_of_memcpy_rate": round(g["pool_read_GBs"] / h2d_rate, 4) if g.get("pool_read_GBs") else None}
         if name in ("lwm_50k", "gqa_128k_host"):   # f4 over a long HBM history and over the host pool
             overlap[name] = measure_overlap(w, lambda fn, n: timed_fn(fn, n, w.sess.compute_stream), 2 if host else 4)
@@ -848,6 +866,18 @@ def run_sweep(args, device, timed, profile, pk, local, timed_fn, overlap) -> dic
         w.sess.close()
         del w
         torch.cuda.empty_cache()
+        if name == "lwm_50k":
+            # the same workload with block ids in ORDER (the locality best case for the paged reads)
+            w = Workload(name, device, args.engine, args.copy, keep_host_layers=0, sorted_table=True)
+            srt = {}
+            for m, mname in ((STAGED, "staged"), (FUSED, "fused")):
+                for _ in range(3):
+                    w.turn(m)
+                srt[mname] = {"ms_per_turn": round(timed(w, m, 5) / 5, 3)}
+            entry["sorted_table"] = srt
+            w.sess.close()
+            del w
+            torch.cuda.empty_cache()
     return out
 
 
