@@ -252,8 +252,11 @@ sc_attn_mma_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
 }
 
 // ------------------------------------------------------------------ combine (a7)
-// One warp per (row, head): O = sum_s 2^(m_s-M) O_s / sum_s 2^(m_s-M) l_s.
-template <int D>
+// One warp per (row, head): O = sum_s 2^(m_s-M) O_s / sum_s 2^(m_s-M) l_s, splits in order.
+// HALF: the partial rows are fp16 scaled by a power of two (the tcgen05 engine: m carries the exponent,
+// l the scaled sum), else fp32 (the mma.sync engine).  Lane sp holds (m, l) of split sp; the O rows of
+// four splits are requested before the first is used.
+template <int D, bool HALF>
 __global__ void __launch_bounds__(256)
 sc_combine_kernel(ScGeom g, ScBatch b, ScAttnArgs a, int tile_m, int split_unit)
 {
@@ -269,24 +272,55 @@ sc_combine_kernel(ScGeom g, ScBatch b, ScAttnArgs a, int tile_m, int split_unit)
     const int rows_valid = min(tile_m, n_s - mt * tile_m);
     const int kmax = b.hist[s] + mt * tile_m + rows_valid;
     const int units_needed = (kmax + split_unit - 1) / split_unit;
-    const int ns = (units_needed + a.split_units - 1) / a.split_units;
-    constexpr int V = D / 32;                                  // floats per lane
-    float M = -INFINITY;
-    for (int sp = 0; sp < ns; ++sp)
-        M = fmaxf(M, a.part_ml[(((int64_t)sp * a.total_new + grow) * g.Hq + h) * 2]);
+    const int ns = (units_needed + a.split_units - 1) / a.split_units;      // <= 32 (max_splits)
+    constexpr int V = D / 32;                                  // values per lane
+    auto prow_of = [&](int sp) { return ((int64_t)sp * a.total_new + grow) * g.Hq + h; };
+    float my_m = -INFINITY, my_l = 0.f;
+    if (lane < ns) {
+        const float2 ml = *reinterpret_cast<const float2 *>(a.part_ml + prow_of(lane) * 2);
+        my_m = ml.x; my_l = ml.y;
+    }
+    float M = my_m;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+    const float my_w = (my_m == -INFINITY) ? 0.f : exp2f(my_m - M);
     float acc[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) acc[v] = 0.f;
     float W = 0.f;
-    for (int sp = 0; sp < ns; ++sp) {
-        const int64_t prow = ((int64_t)sp * a.total_new + grow) * g.Hq + h;
-        const float m = a.part_ml[prow * 2], l = a.part_ml[prow * 2 + 1];
-        const float wgt = (m == -INFINITY) ? 0.f : exp2f(m - M);
-        if (wgt == 0.f) continue;                  // O_s of such a split may never have been written
-        W += wgt * l;
-        const float *o = a.part_o + prow * D + lane * V;
+    for (int sp0 = 0; sp0 < ns; sp0 += 4) {
+        float o[4][V];
 #pragma unroll
-        for (int v = 0; v < V; ++v) acc[v] += wgt * o[v];
+        for (int q = 0; q < 4; ++q) {
+            const int sp = min(sp0 + q, ns - 1);
+            const float wq = __shfl_sync(0xffffffffu, my_w, sp);
+#pragma unroll
+            for (int v = 0; v < V; ++v) o[q][v] = 0.f;
+            if (sp0 + q < ns && wq != 0.f) {          // O_s of a split of weight 0 may never have been written
+                if (HALF) {
+                    const __half *p = reinterpret_cast<const __half *>(a.part_o) + prow_of(sp) * D + lane * V;
+#pragma unroll
+                    for (int v = 0; v < V; v += 2) {
+                        const float2 f = __half22float2(*reinterpret_cast<const __half2 *>(p + v));
+                        o[q][v] = f.x; o[q][v + 1] = f.y;
+                    }
+                } else {
+                    const float *p = a.part_o + prow_of(sp) * D + lane * V;
+#pragma unroll
+                    for (int v = 0; v < V; ++v) o[q][v] = p[v];
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int sp = sp0 + q;
+            const float wq = __shfl_sync(0xffffffffu, my_w, min(sp, ns - 1)), lq = __shfl_sync(0xffffffffu, my_l, min(sp, ns - 1));
+            if (sp < ns && wq != 0.f) {
+                W += wq * lq;
+#pragma unroll
+                for (int v = 0; v < V; ++v) acc[v] += wq * o[q][v];
+            }
+        }
     }
     const float inv = 1.f / W;
     __nv_bfloat16 *out = (__nv_bfloat16 *)a.out + ((int64_t)grow * g.Hq + h) * D + lane * V;
@@ -327,7 +361,12 @@ cudaError_t sc_launch_combine(const ScGeom &g, const ScBatch &b, const ScAttnArg
     const int64_t warps = (int64_t)a.total_new * g.Hq;
     if (warps == 0) return cudaSuccess;
     const unsigned grid = (unsigned)((warps * 32 + 255) / 256);
-    if (g.D == 128) sc_combine_kernel<128><<<grid, 256, 0, st>>>(g, b, a, tile_m, split_unit);
-    else sc_combine_kernel<64><<<grid, 256, 0, st>>>(g, b, a, tile_m, split_unit);
+    if (a.part_half) {
+        if (g.D == 128) sc_combine_kernel<128, true><<<grid, 256, 0, st>>>(g, b, a, tile_m, split_unit);
+        else sc_combine_kernel<64, true><<<grid, 256, 0, st>>>(g, b, a, tile_m, split_unit);
+    } else {
+        if (g.D == 128) sc_combine_kernel<128, false><<<grid, 256, 0, st>>>(g, b, a, tile_m, split_unit);
+        else sc_combine_kernel<64, false><<<grid, 256, 0, st>>>(g, b, a, tile_m, split_unit);
+    }
     return cudaGetLastError();
 }

@@ -780,8 +780,25 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     }
                 }
             } else {
+                // The partial goes to the scratch buffer for sc_combine_kernel in the same form as in the
+                // cluster exchange below: O scaled per row by a power of two 2^-e so that the largest element
+                // lands in [8192, 16384), rounded to fp16, with (A, L) = (m + e, l * 2^-e) -- half the bytes of
+                // fp32 partials for the kernel that writes them and for the one that reads them.
                 const int64_t prow = ((int64_t)split * a.total_new + grow) * g.Hq + h;
-                float *orow = a.part_o + prow * D;
+                __half *orow = reinterpret_cast<__half *>(a.part_o) + prow * D;
+                float amax = 0.f;
+#pragma unroll
+                for (int c4 = 0; c4 < D / 32; ++c4) {
+                    uint32_t o[32];
+                    tmem_ld32(o_addr + c4 * 32, o);
+                    tmem_ld_wait(o);
+#pragma unroll
+                    for (int c = 0; c < 32; c += 2)
+                        amax = max3(amax, fabsf(__uint_as_float(o[c])), fabsf(__uint_as_float(o[c + 1])));
+                }
+                int e = (int)((__float_as_uint(amax) >> 23) & 0xffu) - 140;
+                e = amax > 0.f ? max(e, -100) : 0;                              // all-zero rows keep e = 0
+                const float scale = __uint_as_float((uint32_t)(127 - e) << 23); // 2^-e
 #pragma unroll
                 for (int c4 = 0; c4 < D / 32; ++c4) {
                     uint32_t o[32];
@@ -789,14 +806,17 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     tmem_ld_wait(o);
                     if (valid) {
 #pragma unroll
-                        for (int q4 = 0; q4 < 8; ++q4)
-                            *reinterpret_cast<uint4 *>(orow + c4 * 32 + q4 * 4) =
-                                make_uint4(o[q4 * 4], o[q4 * 4 + 1], o[q4 * 4 + 2], o[q4 * 4 + 3]);
+                        for (int q4 = 0; q4 < 4; ++q4)
+                            *reinterpret_cast<uint4 *>(orow + c4 * 32 + q4 * 8) = make_uint4(
+                                pack_f16(__uint_as_float(o[q4 * 8 + 0]) * scale, __uint_as_float(o[q4 * 8 + 1]) * scale),
+                                pack_f16(__uint_as_float(o[q4 * 8 + 2]) * scale, __uint_as_float(o[q4 * 8 + 3]) * scale),
+                                pack_f16(__uint_as_float(o[q4 * 8 + 4]) * scale, __uint_as_float(o[q4 * 8 + 5]) * scale),
+                                pack_f16(__uint_as_float(o[q4 * 8 + 6]) * scale, __uint_as_float(o[q4 * 8 + 7]) * scale));
                     }
                 }
                 if (valid) {
-                    a.part_ml[prow * 2 + 0] = m_used * sl;      // log2 units; may be -inf
-                    a.part_ml[prow * 2 + 1] = l_run;
+                    a.part_ml[prow * 2 + 0] = m_used * sl + (float)e;      // log2 units; may be -inf
+                    a.part_ml[prow * 2 + 1] = l_run * scale;
                 }
             }
         } else if (a.n_splits > 1 && !a.cluster_combine && r < rows[m]) {

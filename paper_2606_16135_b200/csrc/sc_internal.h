@@ -150,6 +150,7 @@ struct ScAttnArgs {
     ScKvView kv_res;    // staged mode with a regular cache: where logical blocks < rc_blk[s] are read (the pool)
     int32_t has_res;
     float *part_o, *part_ml;
+    int32_t part_half;    // the O partials are fp16 rows scaled by a power of two (tcgen05 engine), else fp32
     // tcgen05 engine: the scatter of the new K/V (a5) is folded into the attention kernel
     const void *k_new, *v_new;   // [sum n][Hkv][D] bf16, or nullptr: already scattered
     ScKvView scat0, scat1;       // where to scatter: the pool, and (staged mode) the LSC

@@ -314,6 +314,7 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     a.kv = lv;
     a.part_o = pool->part_o;
     a.part_ml = pool->part_ml;
+    a.part_half = tc ? 1 : 0;
     a.k_new = fold_scatter ? k_new : nullptr;
     a.v_new = fold_scatter ? v_new : nullptr;
     a.kv_res = pv;
