@@ -264,6 +264,52 @@ sc_status_t sc_prefill_turn_ex(sc_pool_t *pool, const void *q_all, const void *k
                                const int32_t *hist_lens, const int32_t *cu_new, int32_t mode,
                                void *copy_stream, void *compute_stream, const sc_turn_options_t *opt);
 
+/* a5+a6+a7 for callers that must not allocate -- same operation as sc_prefill_layer(FUSED):
+ * scatter, attention over the pool blocks in place, merge
+ * of the split-KV partitions.
+ *
+ * Why it exists.  Everything above needs an sc_pool_t, and sc_pool_create calls cudaMalloc (the
+ * split-KV scratch) and creates streams and events.  Some callers cannot do that: a serving worker
+ * that has already donated every spare byte of HBM to the block pool (PAPER.md:142, :148 -- there is
+ * nothing left to allocate from, the call fails), and any caller on a live GPU that must not stall,
+ * because cudaMalloc / cudaFree wait for the whole device and so hold up every stream on it.  This
+ * call takes no pool object and allocates nothing, on the device or through any library: the partial
+ * (m, l, O) results of the partitions go to a fixed array of SC_STATIC_SCRATCH_BYTES that is part of
+ * the library's device image.  Every GPU on which the library's device code gets loaded holds that
+ * array until the process exits, whether or not this call is ever made again.
+ *
+ * cfg: HOST; only n_layers, n_q_heads, n_kv_heads, head_dim and block_size are read (the geometry
+ * of pool_base, exactly as in sc_pool_create).  pool_base: DEVICE (or peer / mapped pinned host)
+ * pointer to the pool region, 1024-byte aligned; the caller owns it and guarantees it covers every
+ * block id in table_dev.  q, out: DEVICE bf16 [n_new][Hq][D].  k_new, v_new: DEVICE bf16
+ * [n_new][Hkv][D], stored at logical tokens hist_len.. first (rest of the last block zeroed, as
+ * sc_prefill_layer does), or BOTH NULL if those tokens are in the pool already.  table_dev: DEVICE
+ * int32[n_table] covering hist_len + n_new tokens.  Runs on the mma.sync engine.
+ * tiles_per_split: 0 = the library picks the number of partitions and never picks more than fit in
+ * the array; > 0 = that many 64-token KV tiles per partition (as sc_set_split_tiles; at most 32
+ * partitions, longer ranges get larger partitions) -- for equal partitions the output is
+ * bit-identical to sc_prefill_layer's.
+ *
+ * Limit: partitions x n_new x Hq x (D + 2) x 4 bytes (rounded up to 256) must not exceed
+ * SC_STATIC_SCRATCH_BYTES, e.g. 7 partitions of 256 new tokens x 32 heads x D 128.  A forced split
+ * beyond that returns SC_ERR_CAPACITY (message: bytes needed and the limit) and launches nothing;
+ * one partition needs no scratch and always fits.  Other errors as sc_prefill_layer.
+ *
+ * First call on each GPU: looks up the array's device address (cudaGetSymbolAddress, with that GPU
+ * current) and the SM count, and sets one kernel attribute; later calls only launch.  Make that
+ * first call during start-up, outside any stream capture.
+ * Sharing: there is ONE array per GPU for all callers and streams, and it keeps whatever the last
+ * call wrote.  The call never depends on those old contents (every partial the merge reads is
+ * written earlier in the same call, so nothing needs clearing), but two calls whose kernels can
+ * overlap on one GPU -- different streams, different host threads -- race on it and both may
+ * return garbage: issue them on one stream, or order them with events.  Enqueues up to three
+ * kernels on `stream` and returns.                                                           */
+#define SC_STATIC_SCRATCH_BYTES (32u << 20)
+sc_status_t sc_prefill_layer_static(const sc_pool_config_t *cfg, void *pool_base, int32_t layer,
+                                    const void *q, const void *k_new, const void *v_new,
+                                    const int32_t *table_dev, int32_t n_table, int32_t hist_len,
+                                    int32_t n_new, int32_t tiles_per_split, void *out, void *stream);
+
 /* Per-kernel timing for measurement (bench.py's roofline): while enabled, every kernel
  * launch is bracketed by CUDA events on the stream it is launched on.  Enabling clears
  * earlier records.  sc_profile_collect waits for the recorded events and returns, per

@@ -27,6 +27,7 @@ SC_MEM_DEVICE, SC_MEM_HOST_PINNED = 0, 1
 SC_ENGINE_AUTO, SC_ENGINE_MMA_SYNC, SC_ENGINE_TCGEN05 = 0, 1, 2
 SC_COPY_AUTO, SC_COPY_LDG, SC_COPY_BULK = 0, 1, 2
 SC_MAX_SEQS = 32
+SC_STATIC_SCRATCH_BYTES = 32 << 20
 
 STATUS_NAMES = {0: "SC_OK", 1: "SC_ERR_INVALID_ARG", 2: "SC_ERR_OUT_OF_BLOCKS", 3: "SC_ERR_CAPACITY",
                 4: "SC_ERR_BAD_BLOCK_ID", 5: "SC_ERR_CUDA", 6: "SC_ERR_UNSUPPORTED"}
@@ -39,7 +40,7 @@ SYMBOLS = [
     "sc_read_tokens", "sc_load_layer", "sc_prefill_layer", "sc_load_layer_batched",
     "sc_prefill_layer_batched", "sc_prefill_turn", "sc_launch_count", "sc_profile_enable",
     "sc_profile_collect", "sc_lsc_rc_sizing", "sc_elastic_units", "sc_scale_up", "sc_scale_down",
-    "sc_pool_resize", "sc_set_resident_blocks", "sc_prefill_turn_ex",
+    "sc_pool_resize", "sc_set_resident_blocks", "sc_prefill_turn_ex", "sc_prefill_layer_static",
 ]
 
 
@@ -121,6 +122,7 @@ def lib() -> C.CDLL:
         "sc_scale_down": [i64, i32, i64, i64, i64, C.POINTER(i64), C.POINTER(i64)],
         "sc_pool_resize": [vp, i32, sz, i32, vp],
         "sc_set_resident_blocks": [vp, i32],
+        "sc_prefill_layer_static": [C.POINTER(sc_pool_config_t), vp, i32, vp, vp, vp, vp, i32, i32, i32, i32, vp, vp],
     }
     for name, argtypes in sig.items():
         fn = getattr(L, name)
@@ -173,6 +175,19 @@ def sc_scale_down(n_worker_blocks, block_size, meu_worker, meu_master, max_len):
     a, b = C.c_int64(), C.c_int64()
     check(lib().sc_scale_down(n_worker_blocks, block_size, meu_worker, meu_master, max_len, C.byref(a), C.byref(b)))
     return int(a.value), int(b.value)
+
+
+def sc_prefill_layer_static(cfg: sc_pool_config_t, pool_ptr: int, layer: int, q_ptr: int, k_new_ptr: int,
+                            v_new_ptr: int, table_ptr: int, n_table: int, hist_len: int, n_new: int,
+                            tiles_per_split: int, out_ptr: int, stream: int = 0) -> None:
+    """One layer of prefill without a Pool object and without any allocation (see swiftcache.h):
+    for processes that have given all their HBM to the block pool, or that must not stall the GPU
+    with cudaMalloc.  The split-KV partials live in a fixed SC_STATIC_SCRATCH_BYTES array inside the
+    library, ONE per GPU: calls that could overlap on the GPU must be ordered by the caller.
+    ``k_new_ptr`` / ``v_new_ptr`` may both be 0 when the new tokens are in the pool already."""
+    check(lib().sc_prefill_layer_static(C.byref(cfg), pool_ptr or None, layer, q_ptr or None, k_new_ptr or None,
+                                        v_new_ptr or None, table_ptr or None, n_table, hist_len, n_new,
+                                        tiles_per_split, out_ptr or None, stream or None))
 
 
 def make_config(L, Hq, Hkv, D, B, n_blocks, lsc_blocks, max_new_tokens, max_seqs=1,
