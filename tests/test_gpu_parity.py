@@ -244,6 +244,41 @@ def test_pool_and_lsc_prefilled_with_nan(engine, T_h, n, split_tiles):
         c.close()
 
 
+@pytest.mark.parametrize("Hq,T_h,n,split_tiles,what", [
+    (4, 333, 70, 0, "one CTA per pair"),
+    (4, 100, 256, 0, "one CTA per pair, full query pair"),
+    (4, 1000, 255, 2, "forced cluster of 5"),
+    (4, 2049, 130, 3, "forced cluster of 6, second query tile nearly empty"),
+    (32, 5117, 250, 0, "lwm_5k layer shape, the split the heuristic picks"),
+])
+def test_folded_scatter_pads_over_nan_memory(Hq, T_h, n, split_tiles, what):
+    """The headline path: Hq == Hkv and n <= 256, where the tcgen05 kernel stores the new K/V ITSELF
+    (one CTA per pair, or the CTAs of a cluster sharing the rows) and must also zero the rest of the
+    last block -- over a pool and an LSC full of NaN bits, with T_h + n not a multiple of 16.  The
+    launch count proves the scatter kernel did not run; the output must be finite and match the
+    oracle; the written tokens are bit-exact and the tail of the last block reads back as zeros,
+    in the pool and (staged) in the LSC."""
+    assert (T_h + n) % 16 != 0
+    tail = 16 - (T_h + n) % 16
+    for mode in (sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED):
+        c = Case(L=1, Hq=Hq, Hkv=Hq, D=128, T_h=T_h, n=n, NB=400, seed=7300 + T_h, engine=sc.SC_ENGINE_TCGEN05,
+                 split_tiles=split_tiles, zero_fill=False, fill_byte=0xFF)
+        before = c.sess.pool.launch_count()
+        got = c.run_layer(0, mode)
+        launches = c.sess.pool.launch_count() - before
+        assert launches == (2 if mode == sc.SC_ATTN_STAGED else 1), (what, mode, launches)   # (gather +) attention only
+        assert not np.isnan(I.bf16_bits_to_f32(got)).any(), f"NaN in the output: {what}, mode {mode}"
+        assert_close(got, c.oracle_layer(0), f"folded scatter over NaN memory: {what}, mode {mode}")
+        srcs = [0] + ([1] if mode == sc.SC_ATTN_STAGED else [])      # the pool; LSC buffer 0 too when staged
+        for src in srcs:
+            k, v = c.sess.read_tokens(0, src, c.table_dev, 0, T_h + n + tail)
+            k, v = torch_to_bits(k), torch_to_bits(v)
+            assert np.array_equal(k[:T_h + n], np.concatenate([c.data[0][1], c.data[0][3]])), (what, mode, src)
+            assert np.array_equal(v[:T_h + n], np.concatenate([c.data[0][2], c.data[0][4]])), (what, mode, src)
+            assert not k[T_h + n:].any() and not v[T_h + n:].any(), f"tail of the last block not zeroed: {what} src {src}"
+        c.close()
+
+
 # ------------------------------------------------------------------ f2: a pool behind a peer pointer
 def test_peer_pool_kind_routes_like_hbm():
     """the donor pool is another GPU's memory,
