@@ -200,7 +200,21 @@ sc_status_t sc_load_layer(sc_pool_t *pool, int32_t layer, const int32_t *table_d
  *      STAGED reads LSC[buf] (history must have been loaded there), FUSED reads the
  *      pool blocks directly through table_dev and ignores buf;
  *   3. if the history was split across CTAs, the partial (m, l, O) triples are merged.
- * SC_ERR_CAPACITY: table too short, LSC too small (STAGED), n_new > max_new_tokens.    */
+ * SC_ERR_CAPACITY: table too short, LSC too small (STAGED), n_new > max_new_tokens.
+ * Append-only: step 1 treats hist_len + n_new as the END of the conversation.  Whatever the
+ *   last block held behind token hist_len + n_new - 1 (up to 15 tokens) is overwritten with
+ *   zeros, in the pool and in LSC[buf].  Re-running prefill over a middle slice of a
+ *   conversation that is already stored further (recompute, evaluation) therefore destroys
+ *   those tokens' K/V in that block; store them again (sc_store_prefix, which writes exactly
+ *   the tokens it is given and pads nothing) or re-run the later turns.
+ * table_dev (and tables_dev of the batched / turn calls) must be COMPLETE in device memory
+ *   before the kernel that precedes this call on `stream` starts: the tcgen05 engine in FUSED
+ *   mode is launched with programmatic dependent launch and reads the first table entries,
+ *   through the read-only cache, while that preceding kernel may still be running.  A table
+ *   written by a copy or kernel further back in the stream, or before a synchronisation, is
+ *   fine (every use in this repository uploads the table once per turn); a table produced by
+ *   the immediately preceding kernel is not.  q, k_new, v_new and the pool have no such
+ *   restriction: they are read only after the preceding kernel's writes are visible.        */
 sc_status_t sc_prefill_layer(sc_pool_t *pool, int32_t layer, const void *q, const void *k_new,
                              const void *v_new, const int32_t *table_dev, int32_t n_table,
                              int32_t hist_len, int32_t n_new, int32_t buf, int32_t mode,

@@ -385,6 +385,9 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     // Producer warp, lanes 0-7: where block (tile's first block + lane) of this sequence lives.  The
     // block-table read of the FIRST tile is issued here, before the set-up barriers, so that its
     // latency (all CTAs of a launch hit the same table lines at once) is off the critical path.
+    // With a.pdl this read (an __ldg) comes BEFORE griddepcontrol.wait, i.e. possibly while the previous
+    // kernel of the stream still runs: swiftcache.h therefore requires the table to be complete before
+    // that kernel starts.  Everything else the previous kernel may write is read after the wait.
     auto block_ptr = [&](int tb) -> const char * {
         const int lb = min(tb + lane, b_end - 1);
         // a resident block (regular cache) is read in place, the rest from the LSC
