@@ -333,11 +333,30 @@ class Pool:
                         max_blocks, hist_lens, cu_new, mode, copy_stream, compute_stream,
                         lsc_buffers=2, after_attention=None):
         """`after_attention(layer, compute_stream_handle)` is a Python callable run on the host
-        after each layer has been enqueued (it may enqueue work on the compute stream)."""
+        after each layer has been enqueued (it may enqueue work on the compute stream).
+
+        ctypes cannot carry a Python exception through the C frames of the library (it prints it
+        and goes on), so the trampoline keeps the FIRST exception the hook raises, skips the hook
+        for the remaining layers, and this method re-raises it once the C call has returned.  The
+        library has by then enqueued every layer: the turn's own results are complete, only the
+        hook's work is missing from that layer on."""
         h, hp = _i32_array(hist_lens)
         c, cp = _i32_array(cu_new)
-        hook = LAYER_HOOK(lambda layer, stream, user: after_attention(layer, stream)) if after_attention else LAYER_HOOK()
+        raised = []
+
+        def trampoline(layer, stream, user):
+            if raised:
+                return
+            try:
+                after_attention(layer, stream)
+            except BaseException as e:      # noqa: BLE001 -- re-raised below, outside the C frames
+                raised.append(e)
+
+        hook = LAYER_HOOK(trampoline) if after_attention else LAYER_HOOK()
         opt = sc_turn_options_t(lsc_buffers, hook, None)
-        check(lib().sc_prefill_turn_ex(self._h, q_all_ptr, k_all_ptr, v_all_ptr, out_all_ptr, io_kind,
-                                       tables_ptr, max_blocks, len(h), hp, cp, mode, copy_stream or None,
-                                       compute_stream or None, C.byref(opt)))
+        status = lib().sc_prefill_turn_ex(self._h, q_all_ptr, k_all_ptr, v_all_ptr, out_all_ptr, io_kind,
+                                          tables_ptr, max_blocks, len(h), hp, cp, mode, copy_stream or None,
+                                          compute_stream or None, C.byref(opt))
+        if raised:
+            raise raised[0]
+        check(status)

@@ -52,7 +52,8 @@ class Session:
             self.pool_mem = self._pool_owner = None
         self.lsc_mem, self._lsc_owner = _aligned_bytes(max(lsc_bytes, 1024), self.device)
         if fill_byte is not None:          # tests: what the borrowed memory holds before the pool exists
-            self.pool_mem.fill_(fill_byte)
+            if self.pool_mem is not None:  # a region the caller passed in (pool_ptr) is the caller's to fill
+                self.pool_mem.fill_(fill_byte)
             self.lsc_mem.fill_(fill_byte)
         self.pool = sc.Pool(self.cfg, pool_ptr, pool_bytes,
                             self.lsc_mem.data_ptr() if lsc_blocks else 0, lsc_bytes, zero_fill=zero_fill)

@@ -273,6 +273,39 @@ def test_single_buffer_paper_ordering(mode, slow):
     cv.sess.close()
 
 
+def test_an_exception_in_the_layer_hook_reaches_the_caller():
+    """A failing assertion inside after_attention must fail the call that ran it, not vanish on
+    stderr: the binding keeps the hook's first exception, stops calling the hook, lets the library
+    finish enqueuing the turn and re-raises.  The turn itself is still complete and correct."""
+    cv = Conversations(L=4, Hq=4, Hkv=4, D=128, hist=[700], NB=80, max_new=64, seed=29)
+    p, dev = cv.sess.pool, cv.sess.device
+    n_new = [50]
+    cv.begin_turn(n_new)
+    q_all, k_all, v_all = cv.make_inputs(n_new, 912)
+    ref = cv.oracle_turn(q_all, k_all, v_all)
+    tq, tk, tv = (bits_to_torch(x, dev) for x in (q_all, k_all, v_all))
+    out = torch.zeros_like(tq)
+    seen = []
+
+    def hook(layer, stream_handle):
+        seen.append(layer)
+        assert layer != 1, "layer 1 went wrong"
+
+    torch.cuda.synchronize()
+    with pytest.raises(AssertionError, match="layer 1 went wrong"):
+        p.prefill_turn_ex(tq.data_ptr(), tk.data_ptr(), tv.data_ptr(), out.data_ptr(), sc.SC_MEM_DEVICE,
+                          cv.tables_dev.data_ptr(), cv.max_blocks, cv.hist, cv.cu, sc.SC_ATTN_STAGED,
+                          cv.sess.copy_stream.cuda_stream, cv.sess.compute_stream.cuda_stream,
+                          lsc_buffers=1, after_attention=hook)
+    torch.cuda.synchronize()
+    assert seen == [0, 1]                                   # not called again after it failed
+    for l in range(cv.L):
+        assert_close(torch_to_bits(out[l]), ref[l], f"turn with a failing hook: layer {l}")
+    cv.end_turn(n_new)
+    cv.check_pool_equals_logical()
+    cv.sess.close()
+
+
 def test_block_major_resize_on_the_device():
     """f1 (PAPER.md:214-216): growing the pool appends blocks and releasing the tail frees them;
     no existing block moves -- the conversation's KV reads back bit-exactly through the same
