@@ -81,9 +81,9 @@ def _check_turn(w, mode, layers, heads, convs, what):
     torch.cuda.empty_cache()
 
 
-def _workload(name):
+def _workload(name, n_new=None):
     import bench
-    w = bench.Workload(name, torch.device("cuda:0"), keep_host_layers=0)
+    w = bench.Workload(name, torch.device("cuda:0"), keep_host_layers=0, n_new=n_new)
     w._appended = {}
     return w
 
@@ -103,6 +103,52 @@ def test_lwm_50k_sampled():
     L, Hq = w.shape.L, w.shape.Hq
     _check_turn(w, sc.SC_ATTN_FUSED, layers=[0, L - 1], heads=[0, 11, Hq - 1], convs=[0], what="lwm_50k fused")
     _check_turn(w, sc.SC_ATTN_STAGED, layers=[0, 13, L - 1], heads=[0, Hq - 1], convs=[0], what="lwm_50k staged")
+    w.sess.close()
+
+
+@pytest.mark.parametrize("name", ["lwm_5k", "lwm_50k"])
+def test_decode_one_token_at_the_sizes_bench_times(name):
+    """bench.py's `decode` line: n = 1 over the 5 120- and 50 000-token pools, default engine and split
+    heuristic (32 heads x many splits, plain split + merge, ONE valid row per 256-row CTA), staged and
+    fused -- the launch configuration that is timed.  The oracle's cost for one row is nothing, so
+    every head of three layers is compared, and the appended token's bytes are checked in the pool."""
+    w = _workload(name, n_new=1)
+    L, Hq = w.shape.L, w.shape.Hq
+    for mode in (sc.SC_ATTN_FUSED, sc.SC_ATTN_STAGED):
+        _check_turn(w, mode, layers=[0, 13, L - 1], heads=list(range(Hq)), convs=[0], what=f"decode {name} mode {mode}")
+    w.sess.close()
+
+
+def test_lwm_5k_single_buffer_turn_with_busy_hook():
+    """bench.py's `overlap_f4` line at the size it is timed: sc_prefill_turn_ex(lsc_buffers = 1) -- the
+    paper's ordering: load(l+1) into the ONE buffer waits for attention(l) -- over the
+    full lwm_5k turn, with a hook that puts a busy kernel on the compute stream after every attention
+    (what the load is meant to hide behind).  Same sampled rows and pool bytes as the two-buffer test,
+    and the same bits as the two-buffer schedule."""
+    w = _workload("lwm_5k")
+    L, Hq = w.shape.L, w.shape.Hq
+    busy = torch.randn(1024, 1024, device=w.sess.device)
+    seen = []
+
+    def hook(layer, stream_handle):
+        seen.append(layer)
+        with torch.cuda.stream(w.sess.compute_stream):
+            torch.matmul(busy, busy)
+
+    def one_buffer_turn(mode):
+        s = w.sess
+        s.pool.prefill_turn_ex(w.q.data_ptr(), w.k.data_ptr(), w.v.data_ptr(), w.out.data_ptr(), sc.SC_MEM_DEVICE,
+                               w.tables_dev.data_ptr(), w.max_blocks, w.hist, w.cu, mode,
+                               s.copy_stream.cuda_stream, s.compute_stream.cuda_stream,
+                               lsc_buffers=1, after_attention=hook)
+
+    w.turn(sc.SC_ATTN_STAGED)
+    torch.cuda.synchronize()
+    two = w.out.clone()
+    w.turn = one_buffer_turn                   # _check_turn calls w.turn(mode)
+    _check_turn(w, sc.SC_ATTN_STAGED, layers=[0, 11, L - 1], heads=[0, 9, Hq - 1], convs=[0], what="lwm_5k, one LSC buffer")
+    assert seen == list(range(L))
+    assert torch.equal(w.out.view(torch.int16), two.view(torch.int16))
     w.sess.close()
 
 
