@@ -34,12 +34,10 @@
 // the identity table over the LSC.
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
-#include <stdlib.h>
 
 #include <type_traits>
 
 #include "sc_internal.h"
-#include "sc_probe.h"
 
 namespace {
 
@@ -374,8 +372,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     const int ns_act = (need_max + a.split_units - 1) / a.split_units;        // CTAs of the pair that hold keys
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x == 0) { TL(0); TLG(60); }
-    LAUNCH_BEGIN();
     const uint32_t bar_full = smem_u32(&bars->full[0]), bar_empty = smem_u32(&bars->empty[0]);
     const uint32_t bar_s = smem_u32(&bars->s_ready[0]), bar_p = smem_u32(&bars->p_ready[0]);
     const uint32_t bar_q = smem_u32(&bars->q_ready[0]), bar_scat = smem_u32(&bars->scat_done);
@@ -426,7 +422,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
     // up the overlap of the set-up with the previous kernel's tail, 1.18 -> 1.31 ms per fused turn.)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if (threadIdx.x == 128) TL(1);
     float fin_m = -INFINITY, fin_l = 0.f;      // softmax threads: final (m in log2 units, l) of their row
 
     // ---- scatter (a5) ----
@@ -533,11 +528,10 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     const int it = 2 * jj + kv, slot = it % kStages;
                     if (lane == 0) {
                         mbar_wait(bar_empty + 8 * slot, ((it / kStages) & 1) ^ 1);
-                        if (PROBE(4)) mbar_arrive(bar_full + 8 * slot);
-                        else mbar_expect_tx(bar_full + 8 * slot, (uint32_t)nbt * P::kChunk);
+                        mbar_expect_tx(bar_full + 8 * slot, (uint32_t)nbt * P::kChunk);
                     }
                     __syncwarp();
-                    if (lane < nbt && !PROBE(4)) {
+                    if (lane < nbt) {
                         if (LEAN) bulk_g2s_hint(ring + slot * P::kSlot + lane * P::kChunk, blk + off_kv[kv], P::kChunk, bar_full + 8 * slot, pol_stream);
                         else bulk_g2s(ring + slot * P::kSlot + lane * P::kChunk, blk + off_kv[kv], P::kChunk, bar_full + 8 * slot);
                     }
@@ -557,7 +551,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         // =============================== MMA issuer ===============================
         if (lane == 0) {
             auto issue_qk = [&](int m, uint32_t kslot, int nbt) {
-                if (PROBE(3)) return;
                 const uint32_t idesc_qk = make_idesc(16 * nbt, 0);
 #pragma unroll
                 for (int hf = 0; hf < NH; ++hf)
@@ -569,7 +562,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     }
             };
             auto issue_pv = [&](int m, uint32_t vslot, bool acc, int nbt) {
-                if (PROBE(2)) return;
                 constexpr uint32_t idesc_pv = make_idesc(D, 1);
 #pragma unroll
                 for (int kk = 0; kk < kTileBlks; ++kk)             // one MMA consumes one pool block
@@ -659,7 +651,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
                     }
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // before the MMAs read Q and before V of tile 0 lands on the staging slot
                     mbar_arrive(bar_q + 8 * m);
-                    if (threadIdx.x == 128) TL(2);
                 }
             };
             // without a cluster the softmax warps also do the scatter, overlapped with the Q loads
@@ -676,9 +667,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             const int ncols = 16 * min(kTileBlks, b_end - tb);   // keys in this tile
             mbar_wait(bar_s + 8 * m, jj & 1);
             tc_fence_after();
-            if (threadIdx.x == 128 && jj < 12) TL(3 + 2 * jj);
-            if (threadIdx.x == 256 && jj < 12) TL(40 + jj);
-            if (PROBE(1)) { tc_fence_before(); mbar_arrive(bar_p + 8 * m); continue; }
             // last visible column of this row inside the tile; columns past the tile's keys hold
             // stale values, so a tile with fewer than 128 keys is treated as masked
             const int limit = min(T_h + row0 + r - 16 * tb, ncols - 1);
@@ -746,10 +734,8 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&sv[0]));
             if (ncols > 64) tmem_st32(s_addr + 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[32]));
             tmem_st_wait();
-            if (threadIdx.x == 128 && jj == 3) TL(57);
             tc_fence_before();
             mbar_arrive(bar_p + 8 * m);
-            if (threadIdx.x == 128 && jj < 12) TL(4 + 2 * jj);
         }
 
         fin_m = m_used * sl;
@@ -758,7 +744,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         if (nt[m] > 0) {
             mbar_wait(bar_s + 8 * m, nt[m] & 1);
             tc_fence_after();
-            if (threadIdx.x == 128) TL(30);
             const bool valid = r < rows[m];
             if (a.cluster_combine) {
                 // O_m stays in TMEM until the cluster exchange below
@@ -895,7 +880,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // these stores -> the TMA engine's reads
             asm volatile("bar.sync 1, 256;" ::: "memory");                 // the 8 softmax warps
         }
-        if (threadIdx.x == 128) TL(31);
         cluster_wait();                 // every CTA of the cluster is done with its ring and has armed its barrier
         if (threadIdx.x == 128) {
             for (int d = 1; d < ns_act; ++d) {                     // start with the next CTA: spreads the traffic
@@ -911,7 +895,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         }
         if (warp >= 4) {
             mbar_wait_cluster(bar_recv, 0);
-            if (threadIdx.x == 128) TL(32);
         }
         cluster_arrive();               // what this CTA had to receive has landed (so its senders' reads are done)
         if (warp >= 4 && n_mine > 0) {
@@ -975,8 +958,6 @@ sc_attn_tc_kernel(ScGeom g, ScBatch b, ScAttnArgs a)
         cluster_wait();                 // no CTA leaves while a peer's copy may still read its shared memory
     }
 
-    if (threadIdx.x == 128) { TL(33); TLG(61); }
-    LAUNCH_END();
     tc_fence_before();
     __syncthreads();
     if (warp == 2)
@@ -1059,23 +1040,11 @@ int sc_tc_wave_ctas(int D, int lean, int cluster)
     }
     return c > 0 ? c : 0;
 }
-#ifdef SC_TC_PROBE
-extern "C" int sc_probe_read(long long *host) { return (int)cudaMemcpyFromSymbol(host, sc_tl, sizeof(long long) * 256 * 64); }
-extern "C" int sc_probe_read_launches(long long *host) { return (int)cudaMemcpyFromSymbol(host, sc_lt, sizeof(long long) * 256 * 2); }
-#endif
-
 cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st)
 {
     const int total_pairs = b.cu_mt[b.n_seq];
     if (total_pairs == 0) return cudaSuccess;
     dim3 grid((unsigned)a.n_splits, (unsigned)g.Hq, (unsigned)total_pairs);
-#ifdef SC_TC_PROBE
-    {
-        const char *pf = getenv("SC_TC_PROBE");
-        const int flags = pf ? atoi(pf) : 0;
-        cudaMemcpyToSymbolAsync(sc_probe_flags, &flags, sizeof flags, 0, cudaMemcpyHostToDevice, st);
-    }
-#endif
     if (a.has_scat1)   // staged mode: a gather runs beside this kernel
         return g.D == 128 ? launch_tc<128, 1>(g, b, a, grid, st) : launch_tc<64, 1>(g, b, a, grid, st);
     return g.D == 128 ? launch_tc<128, 0>(g, b, a, grid, st) : launch_tc<64, 0>(g, b, a, grid, st);

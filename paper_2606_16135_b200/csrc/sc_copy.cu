@@ -7,7 +7,6 @@
 // 16-byte vectors, coalesced, several independent requests in flight per thread; the
 // bulk variant moves whole pieces with the TMA engine (cp.async.bulk) through a
 // shared-memory ring and keeps the SM's LSU out of it.
-#include <stdlib.h>
 
 #include "sc_internal.h"
 
@@ -264,10 +263,7 @@ cudaError_t sc_launch_gather(const ScGeom &g, const ScBatch &b, const ScKvView &
                                                      cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
                 if (e != cudaSuccess) return e;
             }
-            int grid = n_sms < n_items ? n_sms : n_items;
-#ifdef SC_TC_PROBE
-            if (const char *e = getenv("SC_BULK_GRID")) grid = atoi(e) < n_items ? atoi(e) : n_items;
-#endif
+            const int grid = n_sms < n_items ? n_sms : n_items;
             sc_gather_bulk_kernel<<<grid, 32, smem, st>>>(g, b, src, dst, ppc, piece, n_items);
             return cudaGetLastError();
         }
