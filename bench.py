@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--pool", default="config", choices=["config", "peer"],
                     help="peer (needs --gpus 2): the pool lives on rank 1's GPU, rank 0 reads it over NVLink (f2)")
+    ap.add_argument("--peer-same-gpu", action="store_true",
+                    help="with --pool peer: both ranks on cuda:0, gloo control plane (exercises the IPC path on a 1-GPU box)")
     ap.add_argument("--no-sweep", action="store_true", help="only the headline workload")
     ap.add_argument("--sweep", default=",".join(SWEEP), help="comma-separated workloads measured beside the headline")
     return ap.parse_args()
@@ -432,39 +434,31 @@ def pinned_copy_rates(torch, device, mb=1024) -> tuple:
 
 
 def peer_pool(args, world: int, rank: int, local: int):
-    """with `--gpus 2 --pool peer` the pool region is allocated on rank 1's GPU and
-    opened on rank 0 through CUDA IPC (one process per GPU); rank 0 then runs the workload with
-    pool_kind = SC_POOL_PEER, i.e. every pool read and write crosses NVLink, and rank 1 only lends the
-    memory.  Returns (pointer valid on this rank's device or None, keep-alive objects).
-    UNMEASURED by the builder: it needs two GPUs."""
-    import torch
+    """with `--gpus 2 --pool peer` the pool region is allocated on rank 1's GPU
+    (cudaMalloc, exported through CUDA IPC: paper_2606_16135_b200/peer.py) and opened on rank 0 (one
+    process per GPU); rank 0 then runs the workload with pool_kind = SC_POOL_PEER, i.e. every pool read
+    and write crosses NVLink, and rank 1 only lends the memory.  With --peer-same-gpu both ranks use
+    cuda:0 over a gloo control plane: the same handle / offset / mapping code runs, the link does not.
+    Returns (pointer valid on this rank's device or None, keep-alive object).
+    The NVLink rate is UNMEASURED by the builder: it needs two GPUs."""
     import torch.distributed as dist
-    from cuda import cudart
     from paper_2606_16135_b200 import binding as sc
     from paper_2606_16135_b200 import inputs as I
+    from paper_2606_16135_b200 import peer
     shape = I.configs()[args.workload]
     blocks = sum(-(-(h + shape.n_new * shape.turns) // shape.B) for h in shape.hist)
     cfg = sc.make_config(shape.L, shape.Hq, shape.Hkv, shape.D, shape.B, shape.n_blocks, blocks, shape.n_new)
     pool_bytes, _ = sc.sc_pool_bytes_required(cfg)
-    keep, payload = [], [None]
+    keep, payload = None, [None]
     if rank == 1:
-        mem = torch.zeros(pool_bytes + 1024, dtype=torch.uint8, device=f"cuda:{local}")
-        err, handle = cudart.cudaIpcGetMemHandle(mem.data_ptr())
-        if int(err) != 0:
-            raise SystemExit(f"cudaIpcGetMemHandle: {err}")
-        payload = [(bytes(handle.reserved), mem.data_ptr() % 1024)]
-        keep.append(mem)
+        keep = peer.LentRegion(pool_bytes, device=local)
+        keep.fill(0)
+        payload = [keep.ticket()]
     dist.broadcast_object_list(payload, src=1)
     ptr = None
     if rank == 0:
-        raw, mis = payload[0]
-        h = cudart.cudaIpcMemHandle_t()
-        h.reserved = raw
-        err, base = cudart.cudaIpcOpenMemHandle(h, cudart.cudaIpcMemLazyEnablePeerAccess)
-        if int(err) != 0:
-            raise SystemExit(f"cudaIpcOpenMemHandle: {err} (is there a P2P path between the two GPUs?)")
-        ptr = int(base) + (-(int(base) + 0)) % 1024
-        keep.append(base)
+        keep = peer.OpenedRegion(payload[0], need_bytes=pool_bytes, device=local)
+        ptr = keep.ptr
     return ptr, keep
 
 
@@ -565,8 +559,14 @@ def run_ours(args):
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     if rank == 0:
         sc_build.build()
+    same_gpu = args.pool == "peer" and args.peer_same_gpu
+    if same_gpu:
+        local = 0
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        if same_gpu:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
         dist.barrier()
     device = torch.device(f"cuda:{local}")
     torch.cuda.set_device(device)
@@ -618,6 +618,7 @@ def run_ours(args):
         peer_ptr, peer_keep = peer_pool(args, world, rank, local)
         if rank == 1:                          # lends its memory and waits for rank 0
             dist.barrier()
+            peer_keep.free()                   # rank 0 has closed its mapping by now
             dist.destroy_process_group()
             return
         world = 1                              # one conversation, one compute GPU: no max-over-ranks below
@@ -654,6 +655,20 @@ def run_ours(args):
         w.turn(other_mode)
     o_steps = max(3, min(args.steps, 50))
     other_ms = timed(w, other_mode, o_steps) / o_steps
+
+    # host side of a turn: wall time of the sc_prefill_turn CALL (argument checks, ~2 launches and ~4 event
+    # operations per layer) while the GPU is held up by a sleep kernel, i.e. pure enqueue cost; a turn is
+    # GPU-bound only if this is below its device time
+    host_enqueue = {}
+    for m, mname in ((STAGED, "staged"), (FUSED, "fused")):
+        torch.cuda.synchronize()
+        with torch.cuda.stream(xs):
+            torch.cuda._sleep(int(6e7))                     # ~30 ms at 1.9 GHz: the queue does not drain meanwhile
+        t0 = time.perf_counter()
+        for _ in range(3):
+            w.turn(m)
+        host_enqueue[mname] = round((time.perf_counter() - t0) / 3 * 1e6, 1)
+        torch.cuda.synchronize()
 
     # end to end through the C ABI with HOST buffers (pinned): H2D of q/k/v and D2H of out inside
     e2e = None
@@ -740,12 +755,17 @@ def run_ours(args):
 
     kv_turn_bytes = w.layer_hist_kv_bytes() * shape.L
     job = whole_job(ms_per_step, world, kv_turn_bytes, w.layer_flops() * shape.L)
+    fused_turn_flops = w.layer_flops() * shape.L
+    # what a staged turn must move through HBM at least: the gather's read + write and the attention's read
+    hbm_floor_ms = (w.layer_gather_bytes() + w.layer_hist_kv_bytes()) * shape.L / (pk["hbm_gbs"] * 1e6)
     line = {
-        "metric": METRIC, "value": round(ms_per_step, 4), "unit": "ms", "n_gpus": 2 if peer_ptr else world, "steps": args.steps,
+        "metric": METRIC, "value": round(ms_per_step, 4), "unit": "ms", "n_gpus": (1 if same_gpu else 2) if peer_ptr else world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": config_dict(args.workload, shape, args.mode, world),
-        "pool": ("peer GPU over NVLink (CUDA IPC, SC_POOL_PEER); link rate ~900 GB/s per direction" if peer_ptr else shape.pool_kind),
+        "pool": (("region lent by a second PROCESS on the same GPU (CUDA IPC, SC_POOL_PEER): exercises the mapping, not a link"
+                  if same_gpu else "peer GPU over NVLink (CUDA IPC, SC_POOL_PEER); link rate ~900 GB/s per direction")
+                 if peer_ptr else shape.pool_kind),
         "kv_gbs": round(job["kv_gbs"], 1),
         "attn_tflops": round(job["attn_tflops"], 1),
         "other_mode": {"mode": "fused" if other_mode == FUSED else "staged", "value": round(other_ms, 4),
@@ -754,6 +774,7 @@ def run_ours(args):
         "roofline": roof, "kernels": kernels,
         "isolated": {k: {"avg_ms": round(_avg(v), 5)} for k, v in iso.items() if _avg(v) is not None},
         "cpu_baseline": cpu, "parity": parity,
+        "host_enqueue_us_per_turn": host_enqueue,
     }
     g = _avg(iso["gather"])
     if g:
@@ -774,12 +795,82 @@ def run_ours(args):
         line["sweep"] = run_sweep(args, device, timed, profile, pk, local, timed_fn, line["overlap_f4"])
         line["decode"] = run_decode(args, device, timed, profile, pk)
     if rank == 0:
+        # the driver's record keeps the scalars inside `roofline` and the last ~4 KB of stdout: every figure
+        # DESIGN.md section 9 quotes goes, flat, into both places (`summary` is the LAST key of the line)
+        summary = build_summary(line, pk, fused_turn_flops, hbm_floor_ms)
+        line["roofline"].update(summary)
+        line["summary"] = summary
         print(json.dumps(line))
     if peer_ptr:
+        peer_keep.close()                      # the session over it was closed above
         dist.barrier()                         # releases rank 1
         dist.destroy_process_group()
     elif world > 1:
         dist.destroy_process_group()
+
+
+def build_summary(line: dict, pk: dict, turn_flops: float, hbm_floor_ms: float) -> dict:
+    """Flat scalars (no nesting, < 2 KB) of everything the line measures beside the headline; keys absent
+    where a part did not run.  Fractions: `_frac` of the burst bf16 peak, `_frac_hbm` of the measured
+    copy bandwidth, `_frac_pcie` of a pinned cudaMemcpy measured in the same run."""
+    out = {}
+
+    def put(key, val, nd=4):
+        if val is not None:
+            out[key] = round(float(val), nd)
+
+    def dig(d, *path):
+        for k in path:
+            if not isinstance(d, dict) or k not in d:
+                return None
+            d = d[k]
+        return d
+
+    mode = line["config"].get("mode") if isinstance(line.get("config"), dict) else None
+    staged_ms = line["value"] if mode == "staged" else dig(line, "other_mode", "value")
+    fused_ms = line["value"] if mode == "fused" else dig(line, "other_mode", "value")
+    put("staged_ms", staged_ms)
+    put("fused_ms", fused_ms)
+    if fused_ms:
+        put("fused_frac", turn_flops / fused_ms / 1e9 / pk["bf16_tflops"])
+    if staged_ms:
+        put("step_frac_of_hbm_floor", hbm_floor_ms / staged_ms)
+    put("attention_alone_frac", dig(line, "roofline", "attention_alone", "frac"))
+    put("gather_alone_frac_hbm", dig(line, "isolated", "gather", "frac_of_measured_hbm"))
+    put("gather_in_pipeline_frac_hbm", dig(line, "kernels", "gather", "frac_of_measured_hbm"))
+    put("e2e_ms", dig(line, "e2e", "value"))
+    put("cpu_oracle_ms", dig(line, "cpu_baseline", "value"), 1)
+    put("parity_max_abs", dig(line, "parity", "max_abs"), 6)
+    put("parity_rel_l2", dig(line, "parity", "rel_l2"), 6)
+    sw = line.get("sweep") or {}
+    for name, short in (("lwm_50k", "lwm_50k"), ("gqa_128k", "gqa_128k"), ("multiturn", "multiturn_t0")):
+        for m in ("staged", "fused"):
+            put(f"{short}_{m}_ms", dig(sw, name, m, "ms_per_turn"), 3)
+        put(f"{short}_fused_frac", dig(sw, name, "fused", "kernels", "attention", "frac_of_bf16_burst"))
+        put(f"{short}_gather_in_pipeline_frac_hbm", dig(sw, name, "staged", "kernels", "gather", "frac_of_measured_hbm"))
+    last = [k for k in (sw.get("multiturn") or {}) if k.startswith("turn_")]
+    if last:
+        put("multiturn_last_fused_ms", dig(sw, "multiturn", last[0], "fused", "ms_per_turn"), 3)
+        put("multiturn_last_staged_ms", dig(sw, "multiturn", last[0], "staged", "ms_per_turn"), 3)
+    put("lwm_50k_sorted_fused_ms", dig(sw, "lwm_50k", "sorted_table", "fused", "ms_per_turn"), 3)
+    put("host_pool_staged_ms", dig(sw, "gqa_128k_host", "staged", "ms_per_turn"), 3)
+    put("host_pool_fused_ms", dig(sw, "gqa_128k_host", "fused", "ms_per_turn"), 3)
+    put("host_pool_pcie_gbs", dig(sw, "gqa_128k_host", "pcie", "gather_pool_read_GBs"), 2)
+    put("host_pool_memcpy_gbs", dig(sw, "gqa_128k_host", "pcie", "pinned_memcpy_h2d_GBs"), 2)
+    put("host_pool_frac_pcie", dig(sw, "gqa_128k_host", "pcie", "frac_of_memcpy_rate"))
+    dc = line.get("decode") or {}
+    for name, short in (("lwm_5k", "decode_5k"), ("lwm_50k", "decode_50k")):
+        for m in ("staged", "fused"):
+            put(f"{short}_{m}_ms", dig(dc, name, m, "ms_per_step"))
+            put(f"{short}_{m}_frac_hbm", dig(dc, name, m, "frac_of_measured_hbm"))
+    ov = line.get("overlap_f4") or {}
+    for name, short in (("lwm_5k", "5k"), ("lwm_50k", "50k"), ("gqa_128k_host", "host")):
+        put(f"f4_exposed_pct_{short}", dig(ov, name, "filler", "exposed_load_pct_of_turn"), 2)
+        put(f"f4_single_buffer_ms_{short}", dig(ov, name, "filler", "single_buffer_ms"), 3)
+    he = line.get("host_enqueue_us_per_turn") or {}
+    put("host_enqueue_us_staged", he.get("staged"), 1)
+    put("host_enqueue_us_fused", he.get("fused"), 1)
+    return out
 
 
 def run_decode(args, device, timed, profile, pk) -> dict:

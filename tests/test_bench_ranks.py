@@ -56,3 +56,38 @@ def test_single_rank_needs_no_process_group():
     import bench
     assert bench.max_over_ranks(1.25, 1) == 1.25
     assert bench.whole_job(2.0, 1, 4.0e9, 2.0e12) == {"kv_gbs": 2000.0, "attn_tflops": 1000.0}
+
+
+def test_summary_is_flat_small_and_last():
+    """The driver's record keeps scalars and the tail of stdout: `summary` must be flat numbers,
+    under 2 KB, built from whatever parts of the line exist (absent parts leave no key)."""
+    import json
+    import bench
+    pk = {"hbm_gbs": 6500.0, "bf16_tflops": 1600.0, "bf16_tflops_sustained": 1400.0}
+    line = {"value": 1.7, "config": {"mode": "staged"}, "other_mode": {"mode": "fused", "value": 1.1},
+            "roofline": {"attention_alone": {"frac": 0.31}},
+            "isolated": {"gather": {"frac_of_measured_hbm": 0.78}}, "kernels": {"gather": {"frac_of_measured_hbm": 0.5}},
+            "e2e": {"value": 4.6}, "cpu_baseline": {"value": 25000.0}, "parity": {"max_abs": 1e-4, "rel_l2": 2e-3},
+            "sweep": {"lwm_50k": {"staged": {"ms_per_turn": 9.0, "kernels": {"gather": {"frac_of_measured_hbm": 0.6}}},
+                                  "fused": {"ms_per_turn": 8.2, "kernels": {"attention": {"frac_of_bf16_burst": 0.57}}},
+                                  "sorted_table": {"fused": {"ms_per_turn": 8.1}}},
+                      "multiturn": {"fused": {"ms_per_turn": 20.0}, "turn_9": {"fused": {"ms_per_turn": 23.0}}},
+                      "gqa_128k_host": {"staged": {"ms_per_turn": 343.0}, "pcie": {"gather_pool_read_GBs": 50.2,
+                                        "pinned_memcpy_h2d_GBs": 55.6, "frac_of_memcpy_rate": 0.9}}},
+            "decode": {"lwm_5k": {"fused": {"ms_per_step": 0.88, "frac_of_measured_hbm": 0.39}}},
+            "overlap_f4": {"lwm_5k": {"filler": {"exposed_load_pct_of_turn": 3.5, "single_buffer_ms": 4.2}}},
+            "host_enqueue_us_per_turn": {"staged": 400.0, "fused": 150.0}}
+    s = bench.build_summary(line, pk, turn_flops=7.0e11, hbm_floor_ms=1.2)
+    assert all(isinstance(v, float) for v in s.values())
+    assert len(json.dumps(s)) < 2048
+    assert s["staged_ms"] == 1.7 and s["fused_ms"] == 1.1
+    assert s["fused_frac"] == pytest.approx(7.0e11 / 1.1 / 1e9 / 1600.0, abs=1e-4)
+    assert s["step_frac_of_hbm_floor"] == pytest.approx(1.2 / 1.7, abs=1e-4)
+    assert s["lwm_50k_fused_frac"] == 0.57 and s["multiturn_last_fused_ms"] == 23.0
+    assert s["host_pool_frac_pcie"] == 0.9 and s["decode_5k_fused_frac_hbm"] == 0.39
+    assert s["f4_exposed_pct_5k"] == 3.5 and s["host_enqueue_us_staged"] == 400.0
+    assert "gqa_128k_fused_ms" not in s and "decode_50k_fused_ms" not in s       # parts that did not run
+    # a fused headline swaps the two
+    line["config"]["mode"] = "fused"
+    s = bench.build_summary(line, pk, 7.0e11, 1.2)
+    assert s["fused_ms"] == 1.7 and s["staged_ms"] == 1.1
