@@ -306,6 +306,65 @@ def test_an_exception_in_the_layer_hook_reaches_the_caller():
     cv.sess.close()
 
 
+@pytest.mark.parametrize("mode", [sc.SC_ATTN_STAGED, sc.SC_ATTN_FUSED])
+def test_a_turn_is_capturable_into_a_cuda_graph(mode):
+    """a turn is 32 layers x 2-3 launches plus ~4 event operations per layer
+    from the host; captured once into a CUDA graph it is replayed with ONE launch.  sc_prefill_turn is
+    capturable as it stands once the first (warm-up) turn has set the kernel attributes: it allocates
+    nothing, and the copy stream forks from and joins the compute stream through the pool's events, which
+    is exactly the ordering of PAPER.md:192.  Checked: a replay gives the eager turn's bits, and a replay
+    after the inputs were overwritten in place gives the eager bits and the oracle's values for those."""
+    import copy
+    cv = Conversations(L=5, Hq=4, Hkv=4, D=128, hist=[900, 260], NB=200, max_new=256, seed=41)
+    p, dev = cv.sess.pool, cv.sess.device
+    n_new = [200, 56]
+    cv.begin_turn(n_new)
+    saved = copy.deepcopy(cv.logical)
+    a = cv.make_inputs(n_new, 1201)
+    b = cv.make_inputs(n_new, 1202, variant="peaked")
+    tq, tk, tv = (bits_to_torch(x, dev) for x in a)
+    out = torch.zeros_like(tq)
+    args = (tq.data_ptr(), tk.data_ptr(), tv.data_ptr(), out.data_ptr(), sc.SC_MEM_DEVICE, cv.tables_dev.data_ptr(),
+            cv.max_blocks, cv.hist, cv.cu, mode, cv.sess.copy_stream.cuda_stream, cv.sess.compute_stream.cuda_stream)
+    p.prefill_turn(*args)                                   # eager, inputs A (also the warm-up)
+    torch.cuda.synchronize()
+    eager_a = out.clone()
+    ref_a = cv.oracle_turn(*a)
+    for l in range(cv.L):
+        assert_close(torch_to_bits(eager_a[l]), ref_a[l], f"eager turn, mode {mode}, layer {l}")
+
+    graph = torch.cuda.CUDAGraph()
+    launches_before = p.launch_count()
+    with torch.cuda.graph(graph, stream=cv.sess.compute_stream):
+        p.prefill_turn(*args)
+    captured_launches = p.launch_count() - launches_before
+    assert captured_launches >= cv.L                        # the whole turn went into the graph
+    out.zero_()
+    torch.cuda.synchronize()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out.view(torch.int16), eager_a.view(torch.int16))
+
+    for dst, src in zip((tq, tk, tv), b):                   # new inputs, same addresses
+        dst.copy_(bits_to_torch(src, dev))
+    out.zero_()
+    torch.cuda.synchronize()
+    graph.replay()
+    torch.cuda.synchronize()
+    graph_b = out.clone()
+    p.prefill_turn(*args)
+    torch.cuda.synchronize()
+    assert torch.equal(graph_b.view(torch.int16), out.view(torch.int16))
+    cv.logical = saved                                      # the turn was redone with inputs B over the same slots
+    ref_b = cv.oracle_turn(*b)
+    for l in range(cv.L):
+        assert_close(torch_to_bits(graph_b[l]), ref_b[l], f"graph replay, mode {mode}, layer {l}")
+    cv.end_turn(n_new)
+    cv.check_pool_equals_logical()
+    del graph
+    cv.sess.close()
+
+
 def test_block_major_resize_on_the_device():
     """f1 (PAPER.md:214-216): growing the pool appends blocks and releasing the tail frees them;
     no existing block moves -- the conversation's KV reads back bit-exactly through the same
