@@ -670,6 +670,25 @@ def run_ours(args):
         host_enqueue[mname] = round((time.perf_counter() - t0) / 3 * 1e6, 1)
         torch.cuda.synchronize()
 
+    # the same turn captured once into a CUDA graph and replayed (one launch per turn instead of ~64 launches
+    # and ~130 event operations); same kernels, same ordering (tests/test_gpu_pipeline.py checks the bits)
+    graph_replay = {}
+    for m, mname in ((STAGED, "staged"), (FUSED, "fused")):
+        try:
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr, stream=xs):
+                w.turn(m)
+            g_steps = max(3, min(args.steps, 50))
+            with torch.cuda.stream(xs):                      # a replay goes to torch's current stream
+                for _ in range(3):
+                    gr.replay()
+                graph_replay[mname] = round(timed_fn(gr.replay, g_steps, xs) / g_steps, 4)
+            del gr
+        except Exception as e:                               # noqa: BLE001 -- reported, the headline does not depend on it
+            graph_replay[mname] = None
+            graph_replay[mname + "_error"] = f"{type(e).__name__}: {e}"[:160]
+    torch.cuda.synchronize()
+
     # end to end through the C ABI with HOST buffers (pinned): H2D of q/k/v and D2H of out inside
     e2e = None
     if not args.no_e2e:
@@ -774,7 +793,7 @@ def run_ours(args):
         "roofline": roof, "kernels": kernels,
         "isolated": {k: {"avg_ms": round(_avg(v), 5)} for k, v in iso.items() if _avg(v) is not None},
         "cpu_baseline": cpu, "parity": parity,
-        "host_enqueue_us_per_turn": host_enqueue,
+        "host_enqueue_us_per_turn": host_enqueue, "graph_replay_ms": graph_replay,
     }
     g = _avg(iso["gather"])
     if g:
@@ -870,6 +889,9 @@ def build_summary(line: dict, pk: dict, turn_flops: float, hbm_floor_ms: float) 
     he = line.get("host_enqueue_us_per_turn") or {}
     put("host_enqueue_us_staged", he.get("staged"), 1)
     put("host_enqueue_us_fused", he.get("fused"), 1)
+    gr = line.get("graph_replay_ms") or {}
+    put("graph_replay_staged_ms", gr.get("staged"))
+    put("graph_replay_fused_ms", gr.get("fused"))
     return out
 
 

@@ -75,8 +75,12 @@ typedef enum { SC_POOL_HBM = 0, SC_POOL_HOST_PINNED = 1, SC_POOL_PEER = 2 } sc_p
 typedef enum { SC_ATTN_STAGED = 0, SC_ATTN_FUSED = 1 } sc_attn_mode_t;
 typedef enum { SC_MEM_DEVICE = 0, SC_MEM_HOST_PINNED = 1 } sc_mem_kind_t;
 /* which attention engine sc_prefill_layer* uses; AUTO picks the fastest one
- * that supports the shape */
-typedef enum { SC_ENGINE_AUTO = 0, SC_ENGINE_MMA_SYNC = 1, SC_ENGINE_TCGEN05 = 2 } sc_engine_t;
+ * that supports the shape: SC_ENGINE_DECODE when every conversation of the call brings at most
+ * 16 / (Hq / Hkv) new tokens (decode, n = 1: a paged read of the history, HBM-bound) and the call
+ * reads at least 128 MiB of K/V per layer (below that the tcgen05 kernel's single launch per layer
+ * wins), else SC_ENGINE_TCGEN05.  Forcing SC_ENGINE_DECODE on a call with more rows returns
+ * SC_ERR_UNSUPPORTED. */
+typedef enum { SC_ENGINE_AUTO = 0, SC_ENGINE_MMA_SYNC = 1, SC_ENGINE_TCGEN05 = 2, SC_ENGINE_DECODE = 3 } sc_engine_t;
 /* which copy engine sc_load_layer* uses */
 typedef enum { SC_COPY_AUTO = 0, SC_COPY_LDG = 1, SC_COPY_BULK = 2 } sc_copy_t;
 

@@ -24,7 +24,7 @@ SC_ERR_BAD_BLOCK_ID, SC_ERR_CUDA, SC_ERR_UNSUPPORTED = 4, 5, 6
 SC_POOL_HBM, SC_POOL_HOST_PINNED, SC_POOL_PEER = 0, 1, 2
 SC_ATTN_STAGED, SC_ATTN_FUSED = 0, 1
 SC_MEM_DEVICE, SC_MEM_HOST_PINNED = 0, 1
-SC_ENGINE_AUTO, SC_ENGINE_MMA_SYNC, SC_ENGINE_TCGEN05 = 0, 1, 2
+SC_ENGINE_AUTO, SC_ENGINE_MMA_SYNC, SC_ENGINE_TCGEN05, SC_ENGINE_DECODE = 0, 1, 2, 3
 SC_COPY_AUTO, SC_COPY_LDG, SC_COPY_BULK = 0, 1, 2
 SC_MAX_SEQS = 32
 SC_STATIC_SCRATCH_BYTES = 32 << 20

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libswiftcache.so")
-SOURCES = ["sc_api.cu", "sc_ops.cu", "sc_copy.cu", "sc_attn_mma.cu", "sc_attn_tc.cu", "sc_static.cu"]
+SOURCES = ["sc_api.cu", "sc_ops.cu", "sc_copy.cu", "sc_attn_mma.cu", "sc_attn_tc.cu", "sc_attn_decode.cu", "sc_static.cu"]
 HEADERS = [os.path.join(CSRC, "sc_internal.h"), os.path.join(ROOT, "include", "swiftcache.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",

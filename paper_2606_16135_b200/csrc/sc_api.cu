@@ -241,7 +241,7 @@ sc_status_t sc_lsc_offset(const sc_pool_t *pool, int32_t buf, int32_t lblock, in
 sc_status_t sc_set_engine(sc_pool_t *pool, int32_t attn_engine, int32_t copy_engine)
 {
     if (!pool) return sc_fail(SC_ERR_INVALID_ARG, "pool is NULL");
-    if (attn_engine < SC_ENGINE_AUTO || attn_engine > SC_ENGINE_TCGEN05 || copy_engine < SC_COPY_AUTO ||
+    if (attn_engine < SC_ENGINE_AUTO || attn_engine > SC_ENGINE_DECODE || copy_engine < SC_COPY_AUTO ||
         copy_engine > SC_COPY_BULK)
         return sc_fail(SC_ERR_INVALID_ARG, "unknown engine");
     pool->attn_engine = attn_engine;

@@ -171,5 +171,10 @@ int sc_tc_split_unit();    // tokens per split unit (a pool block)
 int sc_tc_max_cluster();   // most splits the in-kernel (cluster) combine handles
 int sc_tc_wave_ctas(int D, int lean, int cluster);   // co-resident CTAs when launched in clusters of that size
 cudaError_t sc_launch_attn_tc(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st);
+// sc_attn_decode.cu  (decode engine): one CTA per (split, KV head, conversation), at most 16 rows
+int sc_dec_max_rows();     // (new token, query head of the group) rows a CTA holds
+int sc_dec_split_unit();   // tokens per split unit (its 64-token tile)
+int sc_dec_ctas_per_sm();
+cudaError_t sc_launch_attn_decode(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, cudaStream_t st);
 cudaError_t sc_launch_combine(const ScGeom &g, const ScBatch &b, const ScAttnArgs &a, int tile_m,
                               int split_unit, cudaStream_t st);

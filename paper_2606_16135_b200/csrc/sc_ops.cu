@@ -249,9 +249,28 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     if (mode != SC_ATTN_STAGED && mode != SC_ATTN_FUSED) return sc_fail(SC_ERR_INVALID_ARG, "mode %d", mode);
     if (buf < 0 || buf > 1) return sc_fail(SC_ERR_INVALID_ARG, "buf %d not in {0,1}", buf);
     int engine = pool->attn_engine;
-    if (engine == SC_ENGINE_AUTO) engine = SC_ENGINE_TCGEN05;
-    const bool tc = (engine == SC_ENGINE_TCGEN05);
-    const int tile_m = tc ? sc_tc_tile_m() : sc_mma_tile_m(), unit = tc ? sc_tc_split_unit() : sc_mma_split_unit();
+    // A few new tokens per conversation (decode): all rows of a KV head's group fit one 16-row CTA of
+    // the decode engine, which is built for the paged read that is left (sc_attn_decode.cu).
+    bool dec_fits = n_seq > 0 && hist_lens && cu_new;
+    for (int i = 0; dec_fits && i < n_seq; ++i)
+        dec_fits = (int64_t)(cu_new[i + 1] - cu_new[i]) * (pool->g.Hq / pool->g.Hkv) <= sc_dec_max_rows();
+    if (engine == SC_ENGINE_DECODE && !dec_fits)
+        return sc_fail(SC_ERR_UNSUPPORTED, "decode engine: more than %d (new token, query head) rows per KV head",
+                       sc_dec_max_rows());
+    if (engine == SC_ENGINE_AUTO) {
+        // The decode engine costs two more launches per layer (scatter, merge) than the tcgen05 kernel with
+        // its folded scatter and cluster merge, and reads the KV faster: measured cross-over at ~8k tokens
+        // x 32 KV heads x D 128 (27.5 vs 32 us per layer at 5 120 tokens, 194 vs 135 us at 50 000).
+        int64_t kv_bytes = 0;
+        for (int i = 0; dec_fits && i < n_seq; ++i)
+            kv_bytes += ((int64_t)hist_lens[i] + (cu_new[i + 1] - cu_new[i])) * pool->g.Hkv * pool->g.D * 4;
+        const bool long_enough = kv_bytes >= ((int64_t)128 << 20);
+        engine = (dec_fits && long_enough && !(mode == SC_ATTN_STAGED && pool->resident_blocks > 0))
+                     ? SC_ENGINE_DECODE : SC_ENGINE_TCGEN05;
+    }
+    const bool tc = (engine == SC_ENGINE_TCGEN05), dec = (engine == SC_ENGINE_DECODE);
+    const int tile_m = tc ? sc_tc_tile_m() : dec ? sc_dec_max_rows() : sc_mma_tile_m();
+    const int unit = tc ? sc_tc_split_unit() : dec ? sc_dec_split_unit() : sc_mma_split_unit();
     ScBatch b;
     st = make_batch(pool, n_seq, hist_lens, cu_new, max_blocks, tile_m, &b);
     if (st) return st;
@@ -274,7 +293,12 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     for (int i = 0; i < n_seq; ++i)
         max_units = std::max(max_units, ceil_div(hist_lens[i] + (cu_new[i + 1] - cu_new[i]), unit));
     int split_units;
-    if (pool->split_tiles_override <= 0) {
+    if (dec && pool->split_tiles_override <= 0) {
+        // one wave: as many splits as fill every CTA slot of the GPU once
+        const int slots = pool->n_sms * sc_dec_ctas_per_sm(), per_split = pool->g.Hkv * n_seq;
+        const int n_sp = std::max(1, std::min(std::min(slots / per_split, pool->max_splits), max_units));
+        split_units = ceil_div(max_units, n_sp);
+    } else if (pool->split_tiles_override <= 0) {
         const SplitChoice c = choose_split(pool, n_seq, hist_lens, cu_new, tile_m, unit, tc, staged);
         split_units = c.split_units;
         cluster = c.cluster;
@@ -331,7 +355,8 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
     a.total_new = total_new;
     {
         ScProfScope ps(pool, SC_KERNEL_ATTENTION, s);
-        SC_CUDA(tc ? sc_launch_attn_tc(pool->g, b, a, s) : sc_launch_attn_mma(pool->g, b, a, s));
+        SC_CUDA(tc ? sc_launch_attn_tc(pool->g, b, a, s)
+                   : dec ? sc_launch_attn_decode(pool->g, b, a, s) : sc_launch_attn_mma(pool->g, b, a, s));
     }
     pool->launches += 1;
     // 3. combine (a7): with up to 16 splits in one wave the tcgen05 engine merges the partials itself
