@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--mode", default="staged", choices=["staged", "fused"])
     ap.add_argument("--engine", default="auto", choices=["auto", "mma", "tcgen05"])
     ap.add_argument("--copy", default="auto", choices=["auto", "ldg", "bulk"])
+    ap.add_argument("--n-new", type=int, default=None,
+                    help="new tokens per conversation instead of the config's (1 = a decode step); for profiling runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--pool", default="config", choices=["config", "peer"],
@@ -622,7 +624,7 @@ def run_ours(args):
             dist.destroy_process_group()
             return
         world = 1                              # one conversation, one compute GPU: no max-over-ranks below
-    w = Workload(args.workload, device, args.engine, args.copy, peer_pool_ptr=peer_ptr)
+    w = Workload(args.workload, device, args.engine, args.copy, peer_pool_ptr=peer_ptr, n_new=args.n_new)
     shape, pool, xs = w.shape, w.sess.pool, w.sess.compute_stream
     mode = STAGED if args.mode == "staged" else FUSED
 
@@ -740,7 +742,7 @@ def run_ours(args):
         with open(tpath) as f:
             tj = json.load(f)
         traffic = tj.get(f"{args.workload}:{args.mode}:{dom}")
-        traffic_src = tj.get("_source") if traffic is not None else None
+        traffic_src = (tj.get("_source", "") + " | " + tj.get("_commit", "")) if traffic is not None else None
     if bound == "hbm":
         roof = {"kernel": dom, "bound": "hbm", "achieved": round(amount / d_avg / 1e6, 1), "peak": pk["hbm_gbs"],
                 "unit": "GB/s", "peak_source": pk["_source"] + " copy bandwidth"}
@@ -795,6 +797,8 @@ def run_ours(args):
         "cpu_baseline": cpu, "parity": parity,
         "host_enqueue_us_per_turn": host_enqueue, "graph_replay_ms": graph_replay,
     }
+    if args.n_new:
+        line["config"]["workload"] = workload_string(args.workload, shape, n_new=args.n_new)
     g = _avg(iso["gather"])
     if g:
         line["isolated"]["gather"]["GBs"] = round(w.layer_gather_bytes() / g / 1e6, 1)
@@ -878,7 +882,7 @@ def build_summary(line: dict, pk: dict, turn_flops: float, hbm_floor_ms: float) 
     put("host_pool_memcpy_gbs", dig(sw, "gqa_128k_host", "pcie", "pinned_memcpy_h2d_GBs"), 2)
     put("host_pool_frac_pcie", dig(sw, "gqa_128k_host", "pcie", "frac_of_memcpy_rate"))
     dc = line.get("decode") or {}
-    for name, short in (("lwm_5k", "decode_5k"), ("lwm_50k", "decode_50k")):
+    for name, short in (("lwm_5k", "decode_5k"), ("lwm_50k", "decode_50k"), ("gqa_128k", "decode_gqa_128k")):
         for m in ("staged", "fused"):
             put(f"{short}_{m}_ms", dig(dc, name, m, "ms_per_step"))
             put(f"{short}_{m}_frac_hbm", dig(dc, name, m, "frac_of_measured_hbm"))
@@ -901,7 +905,7 @@ def run_decode(args, device, timed, profile, pk) -> dict:
     import torch
     from paper_2606_16135_b200 import binding as sc
     out = {}
-    for name in ("lwm_5k", "lwm_50k"):
+    for name in ("lwm_5k", "lwm_50k", "gqa_128k"):
         w = Workload(name, device, args.engine, args.copy, keep_host_layers=0, n_new=1)
         e = {"workload": workload_string(name, w.shape, n_new=1)}
         for m, mname in ((sc.SC_ATTN_STAGED, "staged"), (sc.SC_ATTN_FUSED, "fused")):

@@ -106,11 +106,12 @@ def test_lwm_50k_sampled():
     w.sess.close()
 
 
-@pytest.mark.parametrize("name", ["lwm_5k", "lwm_50k"])
+@pytest.mark.parametrize("name", ["lwm_5k", "lwm_50k", "gqa_128k"])
 def test_decode_one_token_at_the_sizes_bench_times(name):
-    """bench.py's `decode` line: n = 1 over the 5 120- and 50 000-token pools, default engine and split
-    heuristic (32 heads x many splits, plain split + merge, ONE valid row per 256-row CTA), staged and
-    fused -- the launch configuration that is timed.  The oracle's cost for one row is nothing, so
+    """bench.py's `decode` line: n = 1 over the 5 120-, 50 000- and (GQA 32/8) 131 072-token pools, default
+    engine choice and split heuristic (lwm_5k: the tcgen05 kernel with ONE valid row per 256-row CTA; the
+    two long ones: the decode engine, one wave of splits + merge), staged and fused -- the launch
+    configuration that is timed.  The oracle's cost for one row is nothing, so
     every head of three layers is compared, and the appended token's bytes are checked in the pool."""
     w = _workload(name, n_new=1)
     L, Hq = w.shape.L, w.shape.Hq
