@@ -246,7 +246,9 @@ sc_status_t sc_prefill_layer_batched(sc_pool_t *pool, int32_t layer, const void 
  * q_all, out_all: [L][sum n_new][Hq][D]; k_all, v_all: [L][sum n_new][Hkv][D], bf16.
  * io_kind (sc_mem_kind_t): SC_MEM_DEVICE = DEVICE pointers; SC_MEM_HOST_PINNED = pinned
  * HOST pointers, in which case each layer's q/k/v are copied host->device and its out
- * device->host inside the call (double-buffered staging owned by the library).
+ * device->host inside the call (double-buffered staging owned by the library: allocated ONCE,
+ * by the first such call, for max_new_tokens -- 2 x max_new_tokens x (2 Hq + 2 Hkv) x D x 2
+ * bytes; no later call allocates).
  * mode FUSED skips the loads.  On return all work is enqueued; compute_stream has been
  * made to wait for everything (synchronise it to wait for the turn).                   */
 sc_status_t sc_prefill_turn(sc_pool_t *pool, const void *q_all, const void *k_all,

@@ -415,17 +415,21 @@ sc_status_t sc_prefill_turn_ex(sc_pool_t *pool, const void *q_all, const void *k
     const int L = g.L, total_new = cu_new[n_seq];
     const int64_t q_bytes = (int64_t)total_new * g.Hq * g.D * 2, kv_bytes = (int64_t)total_new * g.Hkv * g.D * 2;
     const bool host_io = (io_kind == SC_MEM_HOST_PINNED);
-    if (host_io) {
-        const int64_t need = 2 * q_bytes + 2 * kv_bytes;   // q, out, k, v
-        if (pool->stage_bytes < need) {
-            for (int i = 0; i < 2; ++i) {
-                if (pool->stage[i]) cudaFree(pool->stage[i]);
+    if (host_io && pool->stage_bytes == 0) {
+        // Allocated ONCE, by the first host-I/O turn, for the largest turn the pool accepts (max_new_tokens):
+        // q, out, k, v of one layer, two slots.  No later call allocates or frees (cudaMalloc / cudaFree
+        // synchronise the device, and a turn that allocates cannot be captured into a graph).
+        const int64_t mt = pool->cfg.max_new_tokens;
+        const int64_t need = 2 * mt * g.Hq * g.D * 2 + 2 * mt * g.Hkv * g.D * 2;
+        for (int i = 0; i < 2; ++i) {
+            cudaError_t e = cudaMalloc((void **)&pool->stage[i], (size_t)need);
+            if (e != cudaSuccess) {
+                if (i == 1) { cudaFree(pool->stage[0]); pool->stage[0] = nullptr; }
                 pool->stage[i] = nullptr;
+                return sc_cuda_fail(e, "cudaMalloc(host-I/O staging)");
             }
-            pool->stage_bytes = 0;
-            for (int i = 0; i < 2; ++i) SC_CUDA(cudaMalloc((void **)&pool->stage[i], (size_t)need));
-            pool->stage_bytes = need;
         }
+        pool->stage_bytes = need;
     }
     // fork: the side streams start after whatever the compute stream already holds
     SC_CUDA(cudaEventRecord(pool->ev_fork, xs));
