@@ -886,6 +886,8 @@ def build_summary(line: dict, pk: dict, turn_flops: float, hbm_floor_ms: float) 
         for m in ("staged", "fused"):
             put(f"{short}_{m}_ms", dig(dc, name, m, "ms_per_step"))
             put(f"{short}_{m}_frac_hbm", dig(dc, name, m, "frac_of_measured_hbm"))
+    put("decode_5k_forced_decode_engine_ms", dig(dc, "lwm_5k", "fused_decode_engine_forced", "ms_per_step"))
+    put("decode_5k_forced_decode_engine_frac_hbm", dig(dc, "lwm_5k", "fused_decode_engine_forced", "frac_of_measured_hbm"))
     ov = line.get("overlap_f4") or {}
     for name, short in (("lwm_5k", "5k"), ("lwm_50k", "50k"), ("gqa_128k_host", "host")):
         put(f"f4_exposed_pct_{short}", dig(ov, name, "filler", "exposed_load_pct_of_turn"), 2)
@@ -919,6 +921,18 @@ def run_decode(args, device, timed, profile, pk) -> dict:
                         "attention_avg_ms": round(att, 5) if att else None,
                         "attention_kv_read_GBs": round(w.layer_hist_kv_bytes() / att / 1e6, 1) if att else None,
                         "frac_of_measured_hbm": round(w.layer_hist_kv_bytes() / att / 1e6 / pk["hbm_gbs"], 4) if att else None}
+        if name == "lwm_5k":
+            # the evidence behind AUTO's choice at short histories: the decode engine FORCED on the same input
+            # (a faster attention launch, but scatter + merge as separate launches; sc_ops.cu keeps the tcgen05
+            # kernel below 128 MiB of K/V per layer)
+            w.sess.pool.set_engine(sc.SC_ENGINE_DECODE, sc.SC_COPY_AUTO)
+            for _ in range(3):
+                w.turn(sc.SC_ATTN_FUSED)
+            ms = timed(w, sc.SC_ATTN_FUSED, 20) / 20
+            att = _avg(profile(w, sc.SC_ATTN_FUSED, 2)["attention"])
+            e["fused_decode_engine_forced"] = {
+                "ms_per_step": round(ms, 4), "attention_avg_ms": round(att, 5) if att else None,
+                "frac_of_measured_hbm": round(w.layer_hist_kv_bytes() / att / 1e6 / pk["hbm_gbs"], 4) if att else None}
         out[name] = e
         w.sess.close()
         del w
